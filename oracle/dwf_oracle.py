@@ -1,0 +1,205 @@
+"""ctypes front-end of the CPU oracle (oracle/dwf_oracle.c).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+import this module.  It never imports the CUDA package.  All arrays are canonical complex128
+(DESIGN.md sec. 3): spinor [nrhs][Ls][t][z][y][x][4][3], gauge [4][t][z][y][x][3][3].
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "dwf_oracle.c")
+_LIB = os.path.join(_HERE, "libdwf_oracle.so")
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (plain -O2, OpenMP over the outer site loop only)."""
+    if force or (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fcx-limited-range", "-fopenmp", "-fPIC", "-shared", "-std=c99",
+               "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.oracle_mpp_inv.restype = ctypes.c_int
+        _lib.oracle_mpc.restype = ctypes.c_int
+        _lib.oracle_cg_schur.restype = ctypes.c_int
+    return _lib
+
+
+def _c(a: np.ndarray) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.complex128)
+
+
+def _p(a: np.ndarray):
+    return a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _L(L):
+    return (ctypes.c_int * 4)(*[int(v) for v in L])
+
+
+def _geom(psi):
+    nrhs, Ls, Lt, Lz, Ly, Lx = psi.shape[:6]
+    return (Lx, Ly, Lz, Lt), Ls, nrhs
+
+
+def gamma(mu: int) -> np.ndarray:
+    """4x4 gamma_mu (mu=0..3) or gamma5 (mu=4) as used by the oracle (R1)."""
+    out = np.zeros((4, 4, 2))
+    lib().oracle_gamma(ctypes.c_int(mu), _p(out))
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def dhop(U, psi, row_parity: int = -1, dagger: bool = False) -> np.ndarray:
+    """D_hop psi (eq. 2)."""
+    psi = _c(psi); U = _c(U); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_dhop(_L(L), ctypes.c_int(Ls), _p(U), _p(psi), _p(out), ctypes.c_int(nrhs),
+                      ctypes.c_int(row_parity), ctypes.c_int(int(dagger)))
+    return out
+
+
+def dwilson(U, psi, M: float) -> np.ndarray:
+    """D_W(M) psi = (M + 4 - D_hop/2) psi (eq. 1), slice by slice."""
+    psi = _c(psi); U = _c(U); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_dwilson(_L(L), ctypes.c_int(Ls), ctypes.c_double(M), _p(U), _p(psi), _p(out),
+                         ctypes.c_int(nrhs))
+    return out
+
+
+def ddw(U, psi, M5: float, mass: float, dagger: bool = False) -> np.ndarray:
+    """D_DW psi (eq. 4, eq. 5); dagger=True is the true adjoint."""
+    psi = _c(psi); U = _c(U); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_ddw(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass), _p(U),
+                     _p(psi), _p(out), ctypes.c_int(nrhs), ctypes.c_int(int(dagger)))
+    return out
+
+
+def dpv(U, psi, M5: float, dagger: bool = False) -> np.ndarray:
+    """D_PV psi = D_DW at unit mass (L50)."""
+    psi = _c(psi); U = _c(U); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_dpv(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), _p(U), _p(psi), _p(out),
+                     ctypes.c_int(nrhs), ctypes.c_int(int(dagger)))
+    return out
+
+
+def gamma5r5(psi) -> np.ndarray:
+    """Gamma5 psi = gamma5 R5 psi (L46)."""
+    psi = _c(psi); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_gamma5r5(_L(L), ctypes.c_int(Ls), _p(psi), _p(out), ctypes.c_int(nrhs))
+    return out
+
+
+def hdw(U, psi, M5: float, mass: float) -> np.ndarray:
+    """H_DW psi = Gamma5 D_DW psi (eq. 6)."""
+    psi = _c(psi); U = _c(U); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_hdw(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass), _p(U),
+                     _p(psi), _p(out), ctypes.c_int(nrhs))
+    return out
+
+
+def mpp(psi, M5: float, mass: float, parity: int, dagger: bool = False) -> np.ndarray:
+    """M_pp psi on sites of `parity` (others 0): the 4D-site-diagonal part of eq. 4."""
+    psi = _c(psi); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_mpp(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass), _p(psi),
+                     _p(out), ctypes.c_int(nrhs), ctypes.c_int(parity), ctypes.c_int(int(dagger)))
+    return out
+
+
+def mpp_inv(psi, M5: float, mass: float, parity: int, dagger: bool = False) -> np.ndarray:
+    """M_pp^{-1} psi by generic dense elimination of the Ls x Ls s-matrix."""
+    psi = _c(psi); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    rc = lib().oracle_mpp_inv(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass),
+                              _p(psi), _p(out), ctypes.c_int(nrhs), ctypes.c_int(parity),
+                              ctypes.c_int(int(dagger)))
+    if rc != 0:
+        raise ZeroDivisionError("M_pp is singular")
+    return out
+
+
+def mpc(U, psi_e, M5: float, mass: float, dagger: bool = False) -> np.ndarray:
+    """Schur operator M_pc = M_ee - M_eo M_oo^{-1} M_oe on an even half field (Table V)."""
+    psi = _c(psi_e); U = _c(U); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    rc = lib().oracle_mpc(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass), _p(U),
+                          _p(psi), _p(out), ctypes.c_int(nrhs), ctypes.c_int(int(dagger)))
+    if rc != 0:
+        raise ZeroDivisionError("M_oo is singular")
+    return out
+
+
+def chebyshev(U, psi, M5: float, mass: float, order: int, lo: float, hi: float) -> np.ndarray:
+    """T_order(2(D^dag D - lo)/(hi-lo) - 1) psi (eq. 23, eq. 34)."""
+    psi = _c(psi); U = _c(U); L, Ls, nrhs = _geom(psi)
+    out = np.empty_like(psi)
+    lib().oracle_chebyshev(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass),
+                           _p(U), ctypes.c_int(order), ctypes.c_double(lo), ctypes.c_double(hi),
+                           _p(psi), _p(out), ctypes.c_int(nrhs))
+    return out
+
+
+def cg_schur(U, b_e, M5: float, mass: float, iters: int, x0=None):
+    """`iters` iterations of CG on M_pc^dag M_pc x = b (eq. 9). Returns (x, |r_k|^2 history)."""
+    b = _c(b_e); U = _c(U); L, Ls, nrhs = _geom(b)
+    assert nrhs == 1
+    x = np.zeros_like(b) if x0 is None else _c(x0).copy()
+    hist = np.zeros(iters + 1)
+    rc = lib().oracle_cg_schur(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass),
+                               _p(U), _p(b), _p(x), ctypes.c_int(iters), _p(hist))
+    if rc != 0:
+        raise ZeroDivisionError("M_oo is singular")
+    return x, hist
+
+
+def inner(x, y) -> np.ndarray:
+    """<x,y> = sum conj(x) y per rhs."""
+    x = _c(x); y = _c(y); nrhs = x.shape[0]
+    out = np.zeros(2 * nrhs)
+    lib().oracle_inner(ctypes.c_int64(x[0].size), ctypes.c_int(nrhs), _p(x), _p(y), _p(out))
+    return out[0::2] + 1j * out[1::2]
+
+
+def norm2(x) -> np.ndarray:
+    return inner(x, x).real
+
+
+def axpy(a, x, y) -> np.ndarray:
+    """y + a x with one complex a per rhs."""
+    x = _c(x); y = _c(y).copy(); nrhs = x.shape[0]
+    a = np.asarray(a, dtype=np.complex128).reshape(nrhs)
+    ab = np.empty(2 * nrhs); ab[0::2] = a.real; ab[1::2] = a.imag
+    lib().oracle_axpy(ctypes.c_int64(x[0].size), ctypes.c_int(nrhs), _p(ab), _p(x), _p(y))
+    return y
+
+
+def ddw_sites(L, Ls: int, M5: float, mass: float, coords, nbr, links) -> np.ndarray:
+    """Site-list mode: D_DW rows at sampled 4D sites from gathered neighbourhoods (see .c header)."""
+    coords = np.ascontiguousarray(coords, dtype=np.int32)
+    n = coords.shape[0]
+    nbr = _c(nbr); links = _c(links)
+    assert nbr.shape == (n, 9, Ls, 4, 3) and links.shape == (n, 8, 3, 3)
+    out = np.empty((n, Ls, 4, 3), dtype=np.complex128)
+    lib().oracle_ddw_sites(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass),
+                           ctypes.c_int64(n), _p(coords), _p(nbr), _p(links), _p(out))
+    return out

@@ -1,0 +1,171 @@
+"""Brute force: the C oracle against dense matrices built from the Kronecker deltas of eq. 2 / eq. 4
+(oracle/dense.py, independent numpy code), on tiny lattices; plus the drivers (Chebyshev, CG)
+against dense eigendecomposition / dense solve, and scalar closed forms of eq. 23 / L173 / Fig. 2.
+"""
+import numpy as np
+import pytest
+
+import dwf_inputs as gen
+from oracle import dense
+
+M5, MASS = 1.8, 0.01
+
+
+def rel(a, b):
+    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+
+
+def test_dense_gammas_match_oracle(oracle):
+    g, g5 = dense.gammas()
+    for mu in range(4):
+        assert np.array_equal(g[mu], oracle.gamma(mu))
+    assert np.array_equal(g5, oracle.gamma(4))
+
+
+def test_dense_wilson_spectrum_free_field():
+    """PAPER.md L69 (4D version): eigenvalues of D_W(M) on unit links are
+    M + 4 - sum cos p_mu +- i sqrt(sum sin^2 p_mu), each 2 (spin) x 3 (colour) fold. Pins dense.py."""
+    L = (4, 2, 2, 4)
+    U = gen.gauge_unit(L)
+    M = -1.8
+    DW = (M + 4) * np.eye(12 * 64) - 0.5 * dense.dhop_4d(U, L)
+    ev = np.linalg.eigvals(DW)
+    want = []
+    for nx in range(L[0]):
+        for ny in range(L[1]):
+            for nz in range(L[2]):
+                for nt in range(L[3]):
+                    p = [2 * np.pi * nx / L[0], 2 * np.pi * ny / L[1], 2 * np.pi * nz / L[2],
+                         2 * np.pi * (nt + 0.5) / L[3]]
+                    # L=2 directions: forward and backward neighbour coincide; the formula still holds
+                    re = M + 4 - sum(np.cos(q) for q in p)
+                    im = np.sqrt(sum(np.sin(q) ** 2 for q in p))
+                    want += [re + 1j * im] * 6 + [re - 1j * im] * 6
+    want = np.array(want)
+    key = lambda v: np.lexsort((np.round(v.imag, 8), np.round(v.real, 8)))
+    assert np.max(np.abs(ev[key(ev)] - want[key(want)])) < 1e-10
+
+
+CASES = [((3, 3, 3, 3), 4), ((4, 2, 2, 2), 4), ((4, 4, 2, 2), 2)]
+
+
+@pytest.mark.parametrize("L,Ls", CASES)
+def test_oracle_vs_dense(oracle, L, Ls):
+    U = gen.gauge_random(L, 5)
+    x = gen.spinor_gaussian(L, Ls, 1, 6)
+    V4 = L[0] * L[1] * L[2] * L[3]
+    xv = x[0].reshape(-1)
+    H4 = dense.dhop_4d(U, L)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    G5 = dense.gamma5r5_5d(L, Ls)
+    # D_hop (every s slice), D_DW, H_DW, D_PV, true adjoints
+    want = (x[0].reshape(Ls, V4 * 12) @ H4.T).reshape(-1)
+    assert rel(oracle.dhop(U, x)[0].reshape(-1), want) < 1e-14
+    want = (x[0].reshape(Ls, V4 * 12) @ H4.conj()).reshape(-1)
+    assert rel(oracle.dhop(U, x, dagger=True)[0].reshape(-1), want) < 1e-14
+    assert rel(oracle.ddw(U, x, M5, MASS)[0].reshape(-1), D @ xv) < 1e-14
+    assert rel(oracle.ddw(U, x, M5, MASS, dagger=True)[0].reshape(-1), D.conj().T @ xv) < 1e-14
+    assert rel(oracle.hdw(U, x, M5, MASS)[0].reshape(-1), G5 @ (D @ xv)) < 1e-14
+    assert rel(oracle.dpv(U, x, M5)[0].reshape(-1), dense.ddw_5d(U, L, Ls, M5, 1.0) @ xv) < 1e-14
+    # dense-level identities: H hermitian (eq. 6), D^dag = Gamma5 D Gamma5 (R12)
+    H = G5 @ D
+    assert np.max(np.abs(H - H.conj().T)) < 1e-14
+    assert np.max(np.abs(G5 @ D @ G5 - D.conj().T)) < 1e-14
+    if all(l % 2 == 0 for l in L):
+        e = dense.parity_mask_5d(L, Ls, 0)
+        Mpc = dense.schur_even(D, L, Ls)
+        xe = gen.keep_parity(x, L, 0)
+        got = oracle.mpc(U, xe, M5, MASS)[0].reshape(-1)
+        assert rel(got[e], Mpc @ xv[e]) < 1e-13
+        assert np.max(np.abs(got[~e])) == 0.0
+        got = oracle.mpc(U, xe, M5, MASS, dagger=True)[0].reshape(-1)
+        assert rel(got[e], Mpc.conj().T @ xv[e]) < 1e-13
+        # M_oo^{-1} against numpy's solve
+        o = ~e
+        xo = gen.keep_parity(x, L, 1)
+        got = oracle.mpp_inv(xo, M5, MASS, 1)[0].reshape(-1)
+        assert rel(got[o], np.linalg.solve(D[np.ix_(o, o)], xv[o])) < 1e-13
+
+
+# ---------------------------------------------------------------- Chebyshev (eq. 23, eq. 34)
+def test_chebyshev_scalar_closed_forms():
+    """T_n(x) = cos(n acos x) (eq. 23), cosh outside; map endpoints (L173); Fig. 2 caption L256:
+    order-500 first pass with lambda_lo = 0.02, lambda_max = 60 enhances low modes by ~1e8."""
+    def T_rec(n, x):
+        t0, t1 = 1.0, x
+        if n == 0:
+            return t0
+        for _ in range(n - 1):
+            t0, t1 = t1, 2 * x * t1 - t0
+        return t1
+    for n in (0, 1, 5, 64):
+        for x in (-1.0, -0.3, 0.0, 0.77, 1.0):
+            assert abs(T_rec(n, x) - np.cos(n * np.arccos(x))) < 1e-12
+    lo, hi = 0.02, 60.0
+    mp = lambda y: 2 * (y - lo) / (hi - lo) - 1
+    assert mp(lo) == -1.0 and abs(mp(hi) - 1.0) < 1e-15
+    val = abs(T_rec(500, mp(0.0)))
+    assert abs(val - np.cosh(500 * np.arccosh(-mp(0.0)))) / val < 1e-9
+    assert 1e7 < val < 1e8            # 4.3e7: "10^8" to the order of magnitude (reading R10)
+
+
+@pytest.mark.parametrize("order", [0, 1, 2, 7, 16])
+def test_chebyshev_vs_eigendecomposition(oracle, order):
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    x = gen.spinor_gaussian(L, Ls, 2, 6)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    lam, V = np.linalg.eigh(D.conj().T @ D)
+    lo, hi = 0.01, 70.0
+    xm = 2 * (lam - lo) / (hi - lo) - 1
+    assert np.all(np.abs(xm) <= 1)
+    Tn = np.cos(order * np.arccos(xm))
+    got = oracle.chebyshev(U, x, M5, MASS, order, lo, hi)
+    for r in range(2):
+        want = V @ (Tn * (V.conj().T @ x[r].reshape(-1)))
+        assert rel(got[r].reshape(-1), want) < 1e-12
+
+
+def test_chebyshev_composition_identity(oracle):
+    """T_2n(X) eta = 2 T_n(X) T_n(X) eta - eta ;  config-level sanity: ||T_64 eta|| / ||eta|| ~ 1/sqrt 2."""
+    L, Ls = (4, 4, 4, 4), 8
+    U = gen.gauge_random(L, 1000)
+    x = gen.spinor_gaussian(L, Ls, 1, 2000)
+    lo, hi = 0.01, 70.0
+    t8 = oracle.chebyshev(U, x, M5, MASS, 8, lo, hi)
+    t16 = oracle.chebyshev(U, x, M5, MASS, 16, lo, hi)
+    assert rel(2 * oracle.chebyshev(U, t8, M5, MASS, 8, lo, hi) - x, t16) < 1e-13
+    t64 = oracle.chebyshev(U, x, M5, MASS, 64, lo, hi)
+    ratio = np.linalg.norm(t64) / np.linalg.norm(x)
+    assert 0.6 < ratio < 0.8
+
+
+# ---------------------------------------------------------------- CG (eq. 9)
+def test_cg_against_dense_solve_and_properties(oracle):
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    b = gen.keep_parity(gen.spinor_gaussian(L, Ls, 1, 6), L, 0)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    e = dense.parity_mask_5d(L, Ls, 0)
+    Mpc = dense.schur_even(D, L, Ls)
+    A = Mpc.conj().T @ Mpc
+    bv = b[0].reshape(-1)[e]
+    x, hist = oracle.cg_schur(U, b, M5, MASS, 150)
+    xs = np.linalg.solve(A, bv)
+    assert rel(x[0].reshape(-1)[e], xs) < 1e-9                       # converges to the dense solution
+    assert abs(hist[0] - np.vdot(bv, bv).real) < 1e-10 * hist[0]     # r_0 = b for x_0 = 0
+    # true residual equals recursive residual; A-norm of the error decreases monotonically
+    errA = []
+    for k in (5, 10, 20, 40):
+        xk, hk = oracle.cg_schur(U, b, M5, MASS, k)
+        xv = xk[0].reshape(-1)[e]
+        true_r = bv - A @ xv
+        assert abs(np.vdot(true_r, true_r).real - hk[k]) < 1e-9 * hk[0]
+        assert np.allclose(hk, hist[:k + 1], rtol=1e-12, atol=0)
+        ev = xv - xs
+        errA.append(np.vdot(ev, A @ ev).real)
+    assert all(errA[i + 1] < errA[i] for i in range(len(errA) - 1))
+    # restart: continuing from x_k reproduces a converging sequence
+    x20, _ = oracle.cg_schur(U, b, M5, MASS, 20)
+    x20b, h2 = oracle.cg_schur(U, b, M5, MASS, 130, x0=x20)
+    assert rel(x20b[0].reshape(-1)[e], xs) < 1e-9
