@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the domain-wall hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+One "step" = one pass of the whole hot path over one batch of seeded synthetic input on the
+16^3 x 32 x Ls=16 fp32 workload (BASELINE.json configs[2]/[3]):
+    a1 import+export (1 field) | a2-a4 D_hop, D_DW, H_DW, D_PV at nrhs=1 and D_DW at nrhs=12, 48 |
+    a5/a6 Schur M_pc on 4 RHS | a7 axpy/inner/norm2 (12 RHS) | a8 order-64 Chebyshev on 24 vectors |
+    a9 20 red-black CG iterations.
+metric = GFlop/s in the standard convention of 1320 flop per 5D site per D_hop-bearing operator
+apply (R20), summed over every apply in the step.  Rank 0 prints ONE JSON line; `detail` carries the
+per-row numbers (D_DW GB/s and GFlop/s per nrhs, Chebyshev vectors/s, CG iterations/s).
+N > 1: independent replicas (the path does not shard: DESIGN.md sec. 8), one process per GPU.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+L = (16, 16, 16, 32)
+LS, M5, MASS = 16, 1.8, 0.01
+V5 = L[0] * L[1] * L[2] * L[3] * LS
+FLOP_PER_SITE = 1320.0
+CHEB_ORDER, CHEB_NVEC, CHEB_LO, CHEB_HI = 64, 24, 0.01, 70.0
+CG_ITERS = 20
+WORKLOAD = "16^3x32xLs16 fp32: D_hop/D_DW/H_DW/D_PV (nrhs 1,12,48) + Schur(4) + BLAS-1 + order-64 Chebyshev(24) + 20 rb-CG it"
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get("hbm_gbs", 6650.0), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def apply_bytes(nrhs: int, real: int = 4) -> float:
+    """Algorithmic bytes of one D_hop/D_DW/H_DW/D_PV apply: 48R + 72R/(Ls nrhs) per 5D site per rhs."""
+    return V5 * nrhs * (48.0 * real + 72.0 * real / (LS * nrhs))
+
+
+def cheb_bytes(order: int, nvec: int, real: int = 4) -> float:
+    """Per order step per 5D site per vector: 6 passes x 24R + 2 gauge reads (D.3)."""
+    return order * (V5 * nvec * 144.0 * real + 2 * (V5 // LS) * 72.0 * real)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            p = [v.strip() for v in r.split(",")]
+            if len(p) < 6:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, p[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_sample(steps: int):
+    """The CPU oracle as it stands on the host cores: `steps` fp64 D_DW applies, nrhs = 1, full volume."""
+    import numpy as np
+    import dwf_inputs as gen
+    from oracle import dwf_oracle as oracle
+    oracle.build()
+    U = gen.gauge_random(L, 1002)
+    psi = gen.spinor_gaussian(L, LS, 1, 2002)
+    oracle.ddw(U, psi[:, :2], M5, MASS)                      # warm the library / OpenMP pool on a thin slice
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        out = oracle.ddw(U, psi, M5, MASS)
+        times.append(time.perf_counter() - t0)
+        psi = out / np.sqrt(np.mean(np.abs(out) ** 2))
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    return times, cores
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (this tier's reference arm)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(1)
+    times, cores = oracle_sample(args.steps)
+    total = sum(times)
+    val = FLOP_PER_SITE * V5 * args.steps / total / 1e9
+    line = {"impl": "reference", "metric": "D_DW-equivalent GFlop/s @1320 flop per 5D site", "value": val, "unit": "GFlop/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": "one fp64 D_DW apply, nrhs=1, full 16^3x32x16 volume per step"},
+            "cpu_baseline": {"value": val, "unit": "GFlop/s", "cores": cores, "kind": "oracle",
+                             "sample": f"{args.steps} fp64 D_DW applies (nrhs=1) on the full 16^3x32x16 volume"},
+            "e2e": {"value": val, "unit": "GFlop/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="dwf", choices=["dwf", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    import dwf_inputs as gen
+    from paper_2103_05034_b200 import (DWF_DDW, DWF_DHOP, DWF_DPV, DWF_F32, DWF_HDW, DWF_SCHUR_EO, Dwf)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+    warmup = max(args.warmup, 3)
+
+    # ---- inputs (seeded, synthetic): SU(3) links from dwf_inputs (host), spinors iid N(0,1)
+    # drawn directly in the native layout by torch's seeded CUDA generator (a permutation of iid Gaussians).
+    d = Dwf(L, LS, M5, MASS, DWF_F32, device=dev)
+    U = torch.from_numpy(gen.gauge_random(L, 1002)).to(torch.complex64).to(dev)
+    d.set_gauge(U)
+    del U
+    d.set_workspace(CHEB_NVEC)
+    g = torch.Generator(device=dev); g.manual_seed(2002 + rank)
+
+    def rnd(nrhs, half=False):
+        f = d.field(nrhs, half=half)
+        f.normal_(generator=g)
+        return f
+
+    NB = 4                                                   # rotate buffers so nrhs=1 applies stream from HBM
+    x1 = [rnd(1) for _ in range(NB)]; y1 = [d.field(1) for _ in range(NB)]
+    x12, y12 = rnd(12), d.field(12)
+    x48, y48 = rnd(48), d.field(48)
+    xs4, ys4 = rnd(4, half=True), d.field(4, half=True)
+    xc, yc = rnd(CHEB_NVEC), d.field(CHEB_NVEC)
+    bcg, xcg = rnd(1, half=True), d.field(1, half=True)
+    canon = torch.randn(d.canonical_shape(1) + (2,), generator=g, device=dev, dtype=torch.float32)
+    canon = torch.view_as_complex(canon).contiguous()
+    host_in = torch.empty(d.canonical_shape(1), dtype=torch.complex64).pin_memory()
+    host_in.copy_(canon.cpu())
+    host_out = torch.empty_like(host_in).pin_memory()
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    parts = {}
+
+    def timed(name, fn):
+        a, b = ev(), ev()
+        a.record(); fn(); b.record()
+        parts.setdefault(name, []).append((a, b))
+
+    hop_applies = {"n": 0.0}
+
+    def step(record):
+        t = timed if record else (lambda name, fn: fn())
+        hop = 0.0
+        t("a1_import_export", lambda: d.export(d.import_(canon, x1[0]), 1, canonical=canon))
+        for i, op in enumerate((DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV)):
+            name = ("dhop", "ddw", "hdw", "dpv")[i] + "_nrhs1"
+            for j in range(NB):
+                t(name, lambda: d.apply(op, x1[j], y1[j], 1))
+            hop += NB
+        t("ddw_nrhs12", lambda: d.apply(DWF_DDW, x12, y12, 12)); hop += 12
+        t("ddw_nrhs48", lambda: d.apply(DWF_DDW, x48, y48, 48)); hop += 48
+        t("schur_nrhs4", lambda: d.apply(DWF_SCHUR_EO, xs4, ys4, 4)); hop += 4
+        t("blas1_nrhs12", lambda: (d.axpy([0.5 + 0.1j] * 12, x12, y12, 12), d.inner(x12, y12, 12), d.norm2(x12, 12)))
+        t("chebyshev", lambda: d.chebyshev(CHEB_ORDER, CHEB_LO, CHEB_HI, xc, yc, CHEB_NVEC)); hop += 2 * CHEB_ORDER * CHEB_NVEC
+        xcg.zero_()
+        t("cg", lambda: d.cg_schur(bcg, xcg, CG_ITERS)); hop += 2 * (CG_ITERS + 1)
+        hop_applies["n"] = hop
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(warmup):
+        step(False)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = d.launch_count()
+    s, e = ev(), ev()
+    s.record()
+    for _ in range(args.steps):
+        step(True)
+    e.record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = d.launch_count() - l0
+    ms = s.elapsed_time(e)
+    if world > 1:
+        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX); ms = float(tt.item())
+        ll = torch.tensor([launches], device=dev, dtype=torch.int64)
+        dist.all_reduce(ll); launches = int(ll.item())
+
+    # ---- e2e: the same apply through the C ABI with HOST buffers (H2D + D2H inside the timed region)
+    for _ in range(2):
+        d.apply_host(DWF_DDW, host_in, host_out, 1)
+    barrier()
+    t0 = time.perf_counter()
+    ne2e = 3
+    for _ in range(ne2e):
+        d.apply_host(DWF_DDW, host_in, host_out, 1)
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / ne2e
+    if world > 1:
+        tt = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX); e2e_s = float(tt.item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    def avg_ms(name):
+        v = [a.elapsed_time(b) for a, b in parts[name]]
+        return sum(v) / len(v)
+
+    peak, peak_src = peaks()
+    detail = {}
+    for name, nrhs in (("dhop_nrhs1", 1), ("ddw_nrhs1", 1), ("hdw_nrhs1", 1), ("dpv_nrhs1", 1), ("ddw_nrhs12", 12), ("ddw_nrhs48", 48)):
+        t_ms = avg_ms(name)
+        detail[name] = {"ms": round(t_ms, 4), "GB/s": round(apply_bytes(nrhs) / t_ms / 1e6, 1),
+                        "GFlop/s": round(FLOP_PER_SITE * V5 * nrhs / t_ms / 1e6, 1),
+                        "frac_of_hbm_peak": round(apply_bytes(nrhs) / t_ms / 1e6 / peak, 4)}
+    t_cheb = avg_ms("chebyshev")
+    detail["chebyshev_order64_24vec"] = {"ms": round(t_cheb, 3), "vectors/s": round(CHEB_NVEC / t_cheb * 1e3, 2),
+                                          "GB/s": round(cheb_bytes(CHEB_ORDER, CHEB_NVEC) / t_cheb / 1e6, 1)}
+    t_cg = avg_ms("cg")
+    detail["rb_cg_16^3x32x16"] = {"ms": round(t_cg, 3), "iterations/s": round((CG_ITERS + 1) / t_cg * 1e3, 1)}
+    for name in ("a1_import_export", "schur_nrhs4", "blas1_nrhs12"):
+        detail[name] = {"ms": round(avg_ms(name), 4)}
+
+    # dominant kernel = hop_kernel inside dwf_chebyshev: 2*order launches per call; its average launch duration
+    # = event-bracketed call time / launches; algorithmic bytes per launch = cheb_bytes / (2*order).
+    n_launch = 2 * CHEB_ORDER
+    ach = cheb_bytes(CHEB_ORDER, CHEB_NVEC) / n_launch / (t_cheb / n_launch) / 1e6
+    roofline = {"bound": "hbm", "kernel": "dwf::hop_kernel<float,...> (H_DW and H_DW+axpby epilogues, nrhs=24, inside dwf_chebyshev)",
+                "achieved": round(ach, 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(ach / peak, 4),
+                "traffic": None, "avg_launch_ms": round(t_cheb / n_launch, 4), "launches_per_step": n_launch,
+                "ddw_nrhs1_frac": detail["ddw_nrhs1"]["frac_of_hbm_peak"]}
+    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(prof):
+        try:
+            roofline["traffic"] = json.load(open(prof)).get("hop_kernel_cheb_bytes_per_launch")
+        except Exception:
+            pass
+
+    total_flop = FLOP_PER_SITE * V5 * hop_applies["n"] * args.steps * world
+    value = total_flop / ms / 1e6
+    e2e_val = FLOP_PER_SITE * V5 * world / e2e_s / 1e9
+    fb = d.field_bytes(1)
+    line = {"metric": "D_DW-equivalent GFlop/s @1320 flop per 5D site", "value": round(value, 1), "unit": "GFlop/s", "n_gpus": world,
+            "steps": args.steps, "warmup": warmup, "ms_per_step": round(ms / args.steps, 3), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "lattice": "16x16x16x32", "Ls": LS, "M5": M5, "mass": MASS,
+                       "l2": "inputs larger than L2 (nrhs>=12 fields >= 2.4 GB); nrhs=1 applies rotate over 4 buffer pairs (1.6 GB)",
+                       "parallelism": "replicas" if world > 1 else "single GPU"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "e2e": {"value": round(e2e_val, 2), "unit": "GFlop/s", "h2d_bytes_per_step": fb, "d2h_bytes_per_step": fb,
+                    "call": "dwf_apply_host(DWF_DDW, nrhs=1): pinned host canonical in -> H2D -> import -> D_DW -> export -> D2H",
+                    "ms": round(e2e_s * 1e3, 3)},
+            "roofline": roofline, "detail": detail}
+    if not args.no_cpu_baseline and world == 1:
+        times, cores = oracle_sample(5)
+        tot = sum(times)
+        line["cpu_baseline"] = {"value": round(FLOP_PER_SITE * V5 * len(times) / tot / 1e9, 3), "unit": "GFlop/s", "cores": cores,
+                                "kind": "oracle", "sample": "5 fp64 D_DW applies (nrhs=1) on the full 16^3x32x16 volume",
+                                "ms_per_apply": round(1e3 * tot / len(times), 1)}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

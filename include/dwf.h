@@ -1,0 +1,122 @@
+/*
+ * dwf.h -- C ABI of libdwf: the data-parallel hot path of arxiv 2103.05034 (Boyle & Yamaguchi,
+ * "Comparison of Domain Wall Fermion Multigrid Methods") as hand-written CUDA for sm_100a (B200).
+ *
+ * What is computed (PAPER.md = /root/reference/PAPER.md line numbers; readings R1..R22 = DESIGN.md sec. 2):
+ *   D_hop      eq. 2  L30   Wilson hopping stencil, spin-projected, SU(3) links
+ *   D_DW       eq. 4  L39 + eq. 5 L43   5D Shamir domain-wall operator
+ *   H_DW       eq. 6  L48   Gamma5 D_DW, Gamma5 = gamma5 R5 (L46)
+ *   D_PV       L50          D_DW at unit mass
+ *   M_pc       Table V L386 even-odd Schur operator M_ee - M_eo M_oo^{-1} M_oe (acts on EVEN half fields)
+ *   Chebyshev  eq. 23, map L173, eq. 34 L227   T_order(2(H_DW^2 - lo)/(hi - lo) - 1)
+ *   rb-CGNR    eq. 9  L73   CG on M_pc^dag M_pc
+ * Conventions: chiral gamma basis (R1), P+- = (1 +- gamma5)/2 (R2), periodic in x,y,z and
+ * antiperiodic in t (R3), 4D red-black parity (x+y+z+t)&1 with even = 0 (R8).
+ *
+ * Pointers: every `const void* / void*` FIELD argument is a DEVICE pointer, 16-byte aligned, owned
+ * by the caller (e.g. a torch tensor's data_ptr); the library never frees or retains it beyond the
+ * call (work is enqueued on the handle's stream; the buffer must stay alive until that work is
+ * done).  Pointers named *_host are HOST pointers.  The handle owns only its gauge copy, its
+ * index tables and a few KB of reduction scratch (cudaMalloc at dwf_create / dwf_set_gauge).
+ *
+ * Layouts.
+ *   canonical spinor : complex<real> [nrhs][Ls][t][z][y][x][spin 4][colour 3], re/im interleaved
+ *   canonical gauge  : complex<real> [mu 4][t][z][y][x][a 3][b 3], mu = 0..3 <-> x,y,z,t,
+ *                      (U psi)_a = sum_b U_ab psi_b
+ *   native spinor    : opaque; dwf_field_bytes() gives its size; a full field is
+ *                      the even half field followed by the odd half field; convert with
+ *                      dwf_import / dwf_export.  `real` is float (DWF_F32) or double (DWF_F64).
+ *
+ * Errors: every int-returning call returns DWF_OK or a negative code and never throws or exits;
+ * dwf_last_error() gives a message.  Calls are asynchronous on the handle's stream unless they
+ * return host values (dwf_inner, dwf_norm2, dwf_cg_schur, dwf_apply_host: these synchronise).
+ * One handle per host thread.
+ */
+#ifndef DWF_H
+#define DWF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dwf_ctx* dwf_handle;
+
+enum { DWF_F32 = 0, DWF_F64 = 1 };
+
+/* Operators for dwf_apply.  Full-field ops: DHOP, DDW, HDW, DPV.  Half-field ops: SCHUR_EO (even
+ * in, even out), MEE (M_ee = M_oo: the 4D-site-diagonal part 5-M5 + fifth-dimension hops of eq. 4)
+ * and MOOINV (its exact inverse, closed form of DESIGN.md sec. 5.4).
+ * OR-ing DWF_DAGGER applies the adjoint (valid for every op; H_DW is hermitian so it is a no-op). */
+enum { DWF_DHOP = 0, DWF_DDW = 1, DWF_HDW = 2, DWF_DPV = 3, DWF_SCHUR_EO = 4, DWF_MEE = 5, DWF_MOOINV = 6,
+       DWF_DAGGER = 0x100 };
+
+enum { DWF_OK = 0, DWF_EINVAL = -1, DWF_ENOGAUGE = -2, DWF_ENOMEM = -3, DWF_ECUDA = -4,
+       DWF_EUNSUPPORTED = -5, DWF_ENOWORKSPACE = -6 };
+
+/* Create a handle.  L = {Lx,Ly,Lz,Lt}, each even and >= 4; Ls even, 2 <= Ls <= 64 (closed-form M_oo^{-1}
+ * is instantiated for Ls in {4,8,12,16,24,32}: other Ls -> DWF_EUNSUPPORTED from SCHUR_EO/MOOINV/CG).
+ * M5 = domain-wall height (eq. 5), mass = m of eq. 4.  M5 == 5 or 1 + m (5-M5)^-Ls == 0 -> DWF_EINVAL
+ * (M_oo singular).  precision: DWF_F32 / DWF_F64 = storage and arithmetic type of fields and links;
+ * reductions always accumulate in fp64.  Uses the current CUDA device. */
+int dwf_create(const int L[4], int Ls, double M5, double mass, int precision, dwf_handle* out);
+int dwf_destroy(dwf_handle h);
+
+/* Stream on which all later work of this handle is enqueued (a cudaStream_t; NULL = default). */
+int dwf_set_stream(dwf_handle h, void* cuda_stream);
+
+/* Scratch for dwf_apply(SCHUR_EO), dwf_chebyshev, dwf_cg_schur, dwf_apply_host with up to `nrhs`
+ * right-hand sides.  The library never allocates field memory: the caller provides a device buffer
+ * of at least dwf_workspace_bytes() bytes and keeps it alive while the handle uses it. */
+size_t dwf_workspace_bytes(dwf_handle h, int nrhs);
+int dwf_set_workspace(dwf_handle h, void* dev_ptr, size_t nbytes);
+
+/* Copy + reorder a canonical gauge field (device pointer, handle precision) into the handle.
+ * The antiperiodic-t sign is folded into the stored U_t on the last time slice.  Stream-ordered. */
+int dwf_set_gauge(dwf_handle h, const void* U_canonical_dev);
+
+/* Bytes of a native field of nrhs right-hand sides; half = 0: full lattice, 1: one parity. */
+size_t dwf_field_bytes(dwf_handle h, int nrhs, int half);
+
+/* canonical (device) <-> native (device).  parity = -1: full field; 0 / 1: the canonical array is a
+ * full-lattice array, only sites of that parity are read (import) / written (export; the other
+ * sites are left untouched), the native buffer is a half field. */
+int dwf_import(dwf_handle h, const void* canonical_dev, void* native_dev, int nrhs, int parity);
+int dwf_export(dwf_handle h, const void* native_dev, void* canonical_dev, int nrhs, int parity);
+
+/* out = OP in, native layout, nrhs fields at once (1 <= nrhs <= 64); in != out. */
+int dwf_apply(dwf_handle h, int op, const void* in, void* out, int nrhs);
+
+/* Same operator, end to end from HOST canonical arrays: H2D copy, import, apply, export, D2H copy
+ * (uses the workspace; synchronises).  For SCHUR_EO/MEE/MOOINV the arrays are full-lattice canonical
+ * arrays of which only the even sites are read and written. */
+int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* out_host, int nrhs);
+
+/* out = T_order(2 (H_DW^2 - lo) / (hi - lo) - 1) in   (eq. 23, eq. 34; R10, R13, R14).
+ * order >= 0, hi > lo.  Full native fields; in != out; uses the workspace (2 full fields). */
+int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, const void* in, void* out, int nrhs);
+
+/* BLAS-1 on native fields (half = 0 full, 1 half field), one scalar per right-hand side.
+ *   axpy : y <- a x + y, a_host[2*nrhs] = (re, im) per rhs
+ *   inner: out_host[2*nrhs] = sum conj(x) y per rhs (fp64 accumulation, deterministic order)
+ *   norm2: out_host[nrhs]   = sum |x|^2 per rhs */
+int dwf_axpy(dwf_handle h, const double* a_host, const void* x, void* y, int nrhs, int half);
+int dwf_inner(dwf_handle h, const void* x, const void* y, double* out_host, int nrhs, int half);
+int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs, int half);
+
+/* `iters` iterations of Hestenes-Stiefel CG on M_pc^dag M_pc x = b (eq. 9), nrhs = 1, even half
+ * fields.  x_even holds x_0 on entry and x_iters on return.  resid2_hist_host (may be NULL) receives
+ * iters+1 values |r_k|^2.  Uses the workspace (5 half fields).  Synchronises at the end only. */
+int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, double* resid2_hist_host);
+
+/* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
+long long dwf_launch_count(dwf_handle h);
+
+/* Message of the last error on this handle (static storage, valid until the next call). */
+const char* dwf_last_error(dwf_handle h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DWF_H */

@@ -1,0 +1,535 @@
+// dwf_api.cu -- host side of libdwf: the C ABI of include/dwf.h, index tables, kernel dispatch and
+// the two drivers (Chebyshev recurrence, red-black CGNR) that only enqueue kernels.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <numeric>
+#include <vector>
+
+#include "../../include/dwf.h"
+#include "dwf_aux.cuh"
+#include "dwf_hop.cuh"
+
+using namespace dwf;
+
+struct dwf_ctx {
+    int L[4], Ls, prec;
+    double M5, mass;
+    long long V4, V4h;
+    cudaStream_t stream;
+    void* gauge;          // native links [2][V4h][4][18] reals
+    int* nbr;             // [2][V4h][8]
+    int* lex;             // [2][V4h]
+    bool have_gauge;
+    void* ws; size_t ws_bytes;
+    double* partial;      // reduction partials [MAX_RED_BLOCKS][64][2]
+    double* scal;         // device scalars (reduction results, CG history)
+    double* scal_host;    // pinned mirror
+    int sm_count;
+    long long launches;
+    char err[256];
+};
+
+static const int MAX_RED_BLOCKS = 2048;
+static const int MAX_NRHS = 64;
+static const int SCAL_DOUBLES = 1 << 16;
+
+#define FAIL(h, code, ...) do { snprintf((h)->err, sizeof((h)->err), __VA_ARGS__); return (code); } while (0)
+#define CUDA_TRY(h, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) \
+    FAIL(h, DWF_ECUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); } while (0)
+#define LAUNCH_CHECK(h) do { (h)->launches++; cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) \
+    FAIL(h, DWF_ECUDA, "kernel launch failed: %s", cudaGetErrorString(e_)); } while (0)
+
+static inline size_t real_bytes(const dwf_ctx* h) { return h->prec == DWF_F32 ? 4 : 8; }
+static inline int vl(const dwf_ctx* h) { return h->prec == DWF_F32 ? 2 : 1; }
+static inline size_t half_bytes(const dwf_ctx* h, int nrhs) {
+    return (size_t)h->V4h * 24 * (size_t)h->Ls * (size_t)nrhs * real_bytes(h);
+}
+static inline long long half_groups(const dwf_ctx* h, int nrhs) {
+    return h->V4h * 12 * ((long long)nrhs * h->Ls / vl(h));
+}
+
+// ------------------------------------------------------------------------------------------------
+// Index tables.  Native site order within a parity: 4D blocks of BLK^4 sites in lexicographic block
+// order, lexicographic inside a block (locality for L1/L2: DESIGN.md sec. 4.1); tables make the order
+// a free choice.  DWF_BLOCK="bx,by,bz,bt" overrides the default.
+// ------------------------------------------------------------------------------------------------
+static void build_tables(const dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nbr) {
+    const int* L = h->L;
+    int B[4] = {4, 4, 4, 4};
+    if (const char* env = getenv("DWF_BLOCK")) {
+        int b[4];
+        if (sscanf(env, "%d,%d,%d,%d", &b[0], &b[1], &b[2], &b[3]) == 4) for (int i = 0; i < 4; i++) B[i] = b[i];
+    }
+    for (int i = 0; i < 4; i++) if (B[i] < 1 || L[i] % B[i] != 0) B[i] = L[i];   // fall back to no blocking
+    if ((B[0] * B[1] * B[2] * B[3]) % 2 != 0) B[0] = L[0];                      // blocks must hold both parities equally
+    const long long V4 = h->V4, V4h = h->V4h;
+    lex.assign(2 * V4h, 0);
+    std::vector<int> idx_of(V4);                                                // lex site -> index within its parity
+    long long cnt[2] = {0, 0};
+    int nb[4]; for (int i = 0; i < 4; i++) nb[i] = L[i] / B[i];
+    for (int bt = 0; bt < nb[3]; bt++) for (int bz = 0; bz < nb[2]; bz++) for (int by = 0; by < nb[1]; by++) for (int bx = 0; bx < nb[0]; bx++)
+        for (int t = bt * B[3]; t < (bt + 1) * B[3]; t++) for (int z = bz * B[2]; z < (bz + 1) * B[2]; z++)
+            for (int y = by * B[1]; y < (by + 1) * B[1]; y++) for (int x = bx * B[0]; x < (bx + 1) * B[0]; x++) {
+                const int p = (x + y + z + t) & 1;
+                const long long lx = x + (long long)L[0] * (y + (long long)L[1] * (z + (long long)L[2] * t));
+                lex[p * V4h + cnt[p]] = (int)lx;
+                idx_of[lx] = (int)cnt[p];
+                cnt[p]++;
+            }
+    nbr.assign(2 * V4h * 8, 0);
+    for (int p = 0; p < 2; p++) for (long long i = 0; i < V4h; i++) {
+        long long lx = lex[p * V4h + i];
+        int c[4]; long long r = lx;
+        for (int d = 0; d < 4; d++) { c[d] = (int)(r % L[d]); r /= L[d]; }
+        for (int mu = 0; mu < 4; mu++) for (int dir = 0; dir < 2; dir++) {
+            int n[4] = {c[0], c[1], c[2], c[3]};
+            n[mu] = (c[mu] + (dir == 0 ? 1 : L[mu] - 1)) % L[mu];
+            const long long nl = n[0] + (long long)L[0] * (n[1] + (long long)L[1] * (n[2] + (long long)L[2] * n[3]));
+            nbr[(p * V4h + i) * 8 + 2 * mu + dir] = idx_of[nl];
+        }
+    }
+}
+
+extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int precision, dwf_handle* out) {
+    if (!out) return DWF_EINVAL;
+    *out = nullptr;
+    if (!L) return DWF_EINVAL;
+    for (int i = 0; i < 4; i++) if (L[i] < 4 || (L[i] & 1)) return DWF_EINVAL;
+    if (Ls < 2 || Ls > 64 || (Ls & 1)) return DWF_EINVAL;
+    if (precision != DWF_F32 && precision != DWF_F64) return DWF_EINVAL;
+    if (M5 == 5.0 || !std::isfinite(M5) || !std::isfinite(mass)) return DWF_EINVAL;
+    if (1.0 + mass * std::pow(5.0 - M5, -(double)Ls) == 0.0) return DWF_EINVAL;
+    const long long V4 = (long long)L[0] * L[1] * L[2] * L[3];
+    if (V4 / 2 * 8 >= (1LL << 31)) return DWF_EUNSUPPORTED;
+    dwf_ctx* h = new (std::nothrow) dwf_ctx();
+    if (!h) return DWF_ENOMEM;
+    memset(h, 0, sizeof(*h));
+    for (int i = 0; i < 4; i++) h->L[i] = L[i];
+    h->Ls = Ls; h->prec = precision; h->M5 = M5; h->mass = mass;
+    h->V4 = V4; h->V4h = V4 / 2;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete h; return DWF_ECUDA;
+    }
+    std::vector<int> lex, nbr;
+    build_tables(h, lex, nbr);
+    const size_t gbytes = (size_t)2 * h->V4h * 72 * real_bytes(h);
+    bool ok = cudaMalloc(&h->gauge, gbytes) == cudaSuccess
+           && cudaMalloc((void**)&h->nbr, nbr.size() * sizeof(int)) == cudaSuccess
+           && cudaMalloc((void**)&h->lex, lex.size() * sizeof(int)) == cudaSuccess
+           && cudaMalloc((void**)&h->partial, (size_t)MAX_RED_BLOCKS * MAX_NRHS * 2 * sizeof(double)) == cudaSuccess
+           && cudaMalloc((void**)&h->scal, SCAL_DOUBLES * sizeof(double)) == cudaSuccess
+           && cudaMallocHost((void**)&h->scal_host, SCAL_DOUBLES * sizeof(double)) == cudaSuccess;
+    ok = ok && cudaMemcpy(h->nbr, nbr.data(), nbr.size() * sizeof(int), cudaMemcpyHostToDevice) == cudaSuccess
+            && cudaMemcpy(h->lex, lex.data(), lex.size() * sizeof(int), cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); dwf_destroy(h); return DWF_ENOMEM; }
+    *out = h;
+    return DWF_OK;
+}
+
+extern "C" int dwf_destroy(dwf_handle h) {
+    if (!h) return DWF_EINVAL;
+    cudaFree(h->gauge); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal);
+    if (h->scal_host) cudaFreeHost(h->scal_host);
+    delete h;
+    return DWF_OK;
+}
+
+extern "C" int dwf_set_stream(dwf_handle h, void* s) { if (!h) return DWF_EINVAL; h->stream = (cudaStream_t)s; return DWF_OK; }
+extern "C" const char* dwf_last_error(dwf_handle h) { return h ? h->err : "null handle"; }
+extern "C" long long dwf_launch_count(dwf_handle h) { return h ? h->launches : -1; }
+
+extern "C" size_t dwf_field_bytes(dwf_handle h, int nrhs, int half) {
+    if (!h || nrhs < 1) return 0;
+    return half ? half_bytes(h, nrhs) : 2 * half_bytes(h, nrhs);
+}
+extern "C" size_t dwf_workspace_bytes(dwf_handle h, int nrhs) {
+    if (!h || nrhs < 1) return 0;
+    return 5 * half_bytes(h, nrhs) + 256;
+}
+extern "C" int dwf_set_workspace(dwf_handle h, void* p, size_t n) {
+    if (!h) return DWF_EINVAL;
+    if (p && ((uintptr_t)p & 15)) FAIL(h, DWF_EINVAL, "workspace must be 16-byte aligned");
+    h->ws = p; h->ws_bytes = p ? n : 0;
+    return DWF_OK;
+}
+static int need_ws(dwf_ctx* h, size_t bytes) {
+    if (!h->ws || h->ws_bytes < bytes)
+        FAIL(h, DWF_ENOWORKSPACE, "workspace of %zu bytes needed, %zu set (dwf_set_workspace)", bytes, h->ws_bytes);
+    return DWF_OK;
+}
+static int check_field(dwf_ctx* h, const void* p, const char* name) {
+    if (!p) FAIL(h, DWF_EINVAL, "%s is NULL", name);
+    if ((uintptr_t)p & 15) FAIL(h, DWF_EINVAL, "%s is not 16-byte aligned", name);
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+extern "C" int dwf_set_gauge(dwf_handle h, const void* U) {
+    if (!h) return DWF_EINVAL;
+    if (int rc = check_field(h, U, "U_canonical_dev")) return rc;
+    const long long n = 2 * h->V4h * 36;
+    const long long spatial = (long long)h->L[0] * h->L[1] * h->L[2];
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    if (h->prec == DWF_F32) reorder_gauge_kernel<float><<<blocks, 256, 0, h->stream>>>((const float*)U, (float*)h->gauge, h->lex, h->V4h, h->V4, spatial, h->L[3]);
+    else                    reorder_gauge_kernel<double><<<blocks, 256, 0, h->stream>>>((const double*)U, (double*)h->gauge, h->lex, h->V4h, h->V4, spatial, h->L[3]);
+    LAUNCH_CHECK(h);
+    h->have_gauge = true;
+    return DWF_OK;
+}
+
+template <typename R, bool IMPORT>
+static int reorder_spinor(dwf_ctx* h, const void* canon_in, void* canon_out, void* native, int nrhs, int parity) {
+    using G = typename Prec<R>::G;
+    const long long per_parity = half_groups(h, nrhs);
+    G* n0; G* n1; const int* l0; const int* l1; unsigned ny;
+    if (parity < 0) { n0 = (G*)native; n1 = (G*)native + per_parity; l0 = h->lex; l1 = h->lex + h->V4h; ny = 2; }
+    else            { n0 = n1 = (G*)native; l0 = l1 = h->lex + (size_t)parity * h->V4h; ny = 1; }
+    dim3 grid((unsigned)((per_parity + 255) / 256), ny);
+    reorder_spinor_kernel<R, IMPORT><<<grid, 256, 0, h->stream>>>((const R*)canon_in, (R*)canon_out, n0, n1, l0, l1, h->V4h, h->V4, h->Ls, nrhs);
+    LAUNCH_CHECK(h);
+    return DWF_OK;
+}
+
+extern "C" int dwf_import(dwf_handle h, const void* canonical, void* native, int nrhs, int parity) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS || parity < -1 || parity > 1) FAIL(h, DWF_EINVAL, "bad nrhs/parity");
+    if (int rc = check_field(h, canonical, "canonical")) return rc;
+    if (int rc = check_field(h, native, "native")) return rc;
+    return h->prec == DWF_F32 ? reorder_spinor<float, true>(h, canonical, nullptr, native, nrhs, parity)
+                              : reorder_spinor<double, true>(h, canonical, nullptr, native, nrhs, parity);
+}
+extern "C" int dwf_export(dwf_handle h, const void* native, void* canonical, int nrhs, int parity) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS || parity < -1 || parity > 1) FAIL(h, DWF_EINVAL, "bad nrhs/parity");
+    if (int rc = check_field(h, canonical, "canonical")) return rc;
+    if (int rc = check_field(h, native, "native")) return rc;
+    return h->prec == DWF_F32 ? reorder_spinor<float, false>(h, nullptr, canonical, (void*)native, nrhs, parity)
+                              : reorder_spinor<double, false>(h, nullptr, canonical, (void*)native, nrhs, parity);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Stencil dispatch
+// ------------------------------------------------------------------------------------------------
+enum HopMode { HM_HOP, HM_HOP_SELF, HM_HOP_SELF_G5, HM_HOP_SELF_G5_AXPBY, HM_SELF };
+
+struct HopCall {            // precision-independent description of one launch
+    int mode; bool dag;
+    int nslots, parity0;    // output parities: parity0 (, parity0^1)
+    const void* in_hop[2]; const void* in_self[2]; void* out[2]; const void* y[2]; const void* z[2];
+    double c_hop, mass, ax_a, ax_b, ax_c;
+    int nrhs;
+};
+
+template <typename R>
+static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
+    using G = typename Prec<R>::G;
+    HopArgs<R> a;
+    for (int s = 0; s < 2; s++) {
+        const int p = (k.parity0 + s) & 1;
+        a.in_hop[s] = (const G*)k.in_hop[s]; a.in_self[s] = (const G*)k.in_self[s]; a.out[s] = (G*)k.out[s];
+        a.y[s] = (const G*)k.y[s]; a.z[s] = (const G*)k.z[s];
+        a.nbr[s] = h->nbr + (size_t)p * h->V4h * 8;
+        a.gauge[s] = (const R*)h->gauge + (size_t)s * h->V4h * 72;      // gauge[] is indexed by PARITY
+    }
+    a.V4h = h->V4h; a.Ls = h->Ls; a.nrhs = k.nrhs; a.NLG = k.nrhs * h->Ls / Prec<R>::VL;
+    a.parity0 = k.parity0;
+    a.c_hop = (R)k.c_hop; a.c_diag = (R)(5.0 - h->M5); a.mass = (R)k.mass;
+    a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c;
+    const long long threads = h->V4h * a.NLG;
+    dim3 grid((unsigned)((threads + 127) / 128), k.nslots);
+    cudaStream_t st = h->stream;
+#define HOPK(DAG, HOP, SELF, G5, AX) hop_kernel<R, DAG, HOP, SELF, G5, AX><<<grid, 128, 0, st>>>(a)
+    switch (k.mode) {
+        case HM_HOP:               if (k.dag) HOPK(true, true, false, false, false); else HOPK(false, true, false, false, false); break;
+        case HM_HOP_SELF:          if (k.dag) HOPK(true, true, true, false, false);  else HOPK(false, true, true, false, false); break;
+        case HM_HOP_SELF_G5:       HOPK(false, true, true, true, false); break;
+        case HM_HOP_SELF_G5_AXPBY: HOPK(false, true, true, true, true); break;
+        case HM_SELF:              if (k.dag) HOPK(true, false, true, false, false); else HOPK(false, false, true, false, false); break;
+        default: FAIL(h, DWF_EINVAL, "bad hop mode");
+    }
+#undef HOPK
+    LAUNCH_CHECK(h);
+    return DWF_OK;
+}
+static int launch_hop(dwf_ctx* h, const HopCall& k) {
+    return h->prec == DWF_F32 ? launch_hop_t<float>(h, k) : launch_hop_t<double>(h, k);
+}
+
+template <typename R, bool DAG>
+static int launch_mooinv_t(dwf_ctx* h, const void* in, void* out, int nrhs, double mass) {
+    using G = typename Prec<R>::G;
+    const double kappa = 1.0 / (5.0 - h->M5);
+    const double v0scale = kappa / (1.0 + mass * std::pow(kappa, (double)h->Ls));
+    const long long threads = h->V4h * 12 * nrhs;
+    const unsigned blocks = (unsigned)((threads + 127) / 128);
+#define MOOK(LS) mooinv_kernel<R, LS, DAG><<<blocks, 128, 0, h->stream>>>((const G*)in, (G*)out, h->V4h, nrhs, (R)kappa, (R)mass, (R)v0scale)
+    switch (h->Ls) {
+        case 4: MOOK(4); break;   case 8: MOOK(8); break;   case 12: MOOK(12); break;
+        case 16: MOOK(16); break; case 24: MOOK(24); break; case 32: MOOK(32); break;
+        default: FAIL(h, DWF_EUNSUPPORTED, "M_oo^-1 is instantiated for Ls in {4,8,12,16,24,32}, got %d", h->Ls);
+    }
+#undef MOOK
+    LAUNCH_CHECK(h);
+    return DWF_OK;
+}
+static int launch_mooinv(dwf_ctx* h, const void* in, void* out, int nrhs, double mass, bool dag) {
+    if (h->prec == DWF_F32) return dag ? launch_mooinv_t<float, true>(h, in, out, nrhs, mass) : launch_mooinv_t<float, false>(h, in, out, nrhs, mass);
+    return dag ? launch_mooinv_t<double, true>(h, in, out, nrhs, mass) : launch_mooinv_t<double, false>(h, in, out, nrhs, mass);
+}
+
+// full-lattice operator:  out_p = c_hop hop(in_{1-p}) [+ self(in_p)] for both parities, one launch
+static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, const void* in, void* out, int nrhs,
+                   double ax_a = 0, const void* y = nullptr, double ax_b = 0, const void* z = nullptr, double ax_c = 0) {
+    const size_t hb = half_bytes(h, nrhs);
+    HopCall k{};
+    k.mode = mode; k.dag = dag; k.nslots = 2; k.parity0 = 0; k.nrhs = nrhs;
+    for (int p = 0; p < 2; p++) {
+        k.in_hop[p] = (const char*)in + (size_t)(1 - p) * hb;
+        k.in_self[p] = (const char*)in + (size_t)p * hb;
+        k.out[p] = (char*)out + (size_t)p * hb;
+        k.y[p] = y ? (const char*)y + (size_t)p * hb : nullptr;
+        k.z[p] = z ? (const char*)z + (size_t)p * hb : nullptr;
+    }
+    k.c_hop = c_hop; k.mass = mass; k.ax_a = ax_a; k.ax_b = ax_b; k.ax_c = ax_c;
+    return launch_hop(h, k);
+}
+
+// Schur operator on even half fields:  tmp_o = M_oo^-1 Dhop_oe in ;
+// out = M_ee in - 1/4 Dhop_eo tmp_o     [M_eo = M_oe = -1/2 Dhop].  dag: every factor adjoint.
+static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs) {
+    HopCall k1{};
+    k1.mode = HM_HOP; k1.dag = dag; k1.nslots = 1; k1.parity0 = 1; k1.nrhs = nrhs;
+    k1.in_hop[0] = in; k1.out[0] = tmp; k1.c_hop = 1.0; k1.mass = h->mass;
+    if (int rc = launch_hop(h, k1)) return rc;
+    if (int rc = launch_mooinv(h, tmp, tmp, nrhs, h->mass, dag)) return rc;
+    HopCall k2{};
+    k2.mode = HM_HOP_SELF; k2.dag = dag; k2.nslots = 1; k2.parity0 = 0; k2.nrhs = nrhs;
+    k2.in_hop[0] = tmp; k2.in_self[0] = in; k2.out[0] = out; k2.c_hop = -0.25; k2.mass = h->mass;
+    return launch_hop(h, k2);
+}
+
+static int apply_checked(dwf_ctx* h, int op, const void* in, void* out, int nrhs) {
+    const bool dag = (op & DWF_DAGGER) != 0;
+    const int base = op & ~DWF_DAGGER;
+    switch (base) {
+        case DWF_DHOP: return full_op(h, HM_HOP, dag, 1.0, h->mass, in, out, nrhs);
+        case DWF_DDW:  return full_op(h, HM_HOP_SELF, dag, -0.5, h->mass, in, out, nrhs);
+        case DWF_DPV:  return full_op(h, HM_HOP_SELF, dag, -0.5, 1.0, in, out, nrhs);
+        case DWF_HDW:  return full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, in, out, nrhs);
+        case DWF_SCHUR_EO: {
+            if (int rc = need_ws(h, half_bytes(h, nrhs))) return rc;
+            return schur_op(h, dag, in, out, h->ws, nrhs);
+        }
+        case DWF_MEE: {
+            HopCall k{};
+            k.mode = HM_SELF; k.dag = dag; k.nslots = 1; k.parity0 = 0; k.nrhs = nrhs;
+            k.in_self[0] = in; k.out[0] = out; k.mass = h->mass;
+            return launch_hop(h, k);
+        }
+        case DWF_MOOINV: return launch_mooinv(h, in, out, nrhs, h->mass, dag);
+        default: FAIL(h, DWF_EINVAL, "unknown op %d", op);
+    }
+}
+
+extern "C" int dwf_apply(dwf_handle h, int op, const void* in, void* out, int nrhs) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
+    if (int rc = check_field(h, in, "in")) return rc;
+    if (int rc = check_field(h, out, "out")) return rc;
+    if (in == out) FAIL(h, DWF_EINVAL, "in == out: the stencil is not in-place safe");
+    const int base = op & ~DWF_DAGGER;
+    if (base != DWF_MEE && base != DWF_MOOINV && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    return apply_checked(h, op, in, out, nrhs);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Chebyshev driver:  X = alpha H^2 - beta, alpha = 2/(hi-lo), beta = (hi+lo)/(hi-lo)
+//   t_1 = alpha H(H t_0) - beta t_0 ;  t_{k+1} = 2 alpha H(H t_k) - 2 beta t_k - t_{k-1}
+// Each step = two stencil launches; the second carries the three-term recurrence in its epilogue and
+// overwrites t_{k-1} in place.  Odd t_k live in buffer A, even ones in B; A/B are chosen so that
+// t_order lands in `out`.
+// ------------------------------------------------------------------------------------------------
+extern "C" int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, const void* in, void* out, int nrhs) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
+    if (order < 0 || !(hi > lo)) FAIL(h, DWF_EINVAL, "need order >= 0 and hi > lo");
+    if (int rc = check_field(h, in, "in")) return rc;
+    if (int rc = check_field(h, out, "out")) return rc;
+    if (in == out) FAIL(h, DWF_EINVAL, "in == out");
+    if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    const size_t fb = 2 * half_bytes(h, nrhs);
+    if (order == 0) { CUDA_TRY(h, cudaMemcpyAsync(out, in, fb, cudaMemcpyDeviceToDevice, h->stream)); return DWF_OK; }
+    if (int rc = need_ws(h, 2 * fb)) return rc;
+    void* w = h->ws;
+    void* other = (char*)h->ws + fb;
+    void* A = (order & 1) ? out : other;      // holds t_1, t_3, ...
+    void* B = (order & 1) ? other : out;      // holds t_2, t_4, ...
+    const double alpha = 2.0 / (hi - lo), beta = (hi + lo) / (hi - lo);
+    // t_1 = alpha H H t_0 - beta t_0
+    if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, in, w, nrhs)) return rc;
+    if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, A, nrhs, alpha, in, -beta, in, 0.0)) return rc;
+    const void* tkm1 = in; void* tk = A;
+    for (int k = 1; k < order; k++) {
+        void* dst = (k == 1) ? B : (void*)tkm1;           // t_{k+1} overwrites t_{k-1} (except t_0 = user input)
+        if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, tk, w, nrhs)) return rc;
+        if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, 2.0 * alpha, tk, -2.0 * beta, tkm1, -1.0)) return rc;
+        tkm1 = tk; tk = dst;
+    }
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// BLAS-1
+// ------------------------------------------------------------------------------------------------
+static unsigned blas_blocks(const dwf_ctx* h, long long ngroups, int NLG) {
+    // (blocks * 256) % NLG == 0 so that each thread keeps one rhs over its grid-stride loop
+    const long long unit = NLG / std::gcd((long long)NLG, 256LL);
+    long long want = std::min<long long>((ngroups + 255) / 256, (long long)h->sm_count * 8);
+    long long blocks = std::max<long long>(unit, (want / unit) * unit);
+    if (blocks > MAX_RED_BLOCKS) blocks = std::max<long long>(unit, (MAX_RED_BLOCKS / unit) * unit);
+    return (unsigned)blocks;
+}
+
+static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp) {
+    const long long ng = half_groups(h, nrhs) * (half ? 1 : 2);
+    const int NLG = nrhs * h->Ls / vl(h);
+    const unsigned blocks = blas_blocks(h, ng, NLG);
+    if (h->prec == DWF_F32) {
+        if (norm) inner_kernel<float, true><<<blocks, 256, 0, h->stream>>>((const float4*)x, nullptr, ng, NLG, h->Ls, nrhs, h->partial);
+        else      inner_kernel<float, false><<<blocks, 256, 0, h->stream>>>((const float4*)x, (const float4*)y, ng, NLG, h->Ls, nrhs, h->partial);
+    } else {
+        if (norm) inner_kernel<double, true><<<blocks, 256, 0, h->stream>>>((const double2*)x, nullptr, ng, NLG, h->Ls, nrhs, h->partial);
+        else      inner_kernel<double, false><<<blocks, 256, 0, h->stream>>>((const double2*)x, (const double2*)y, ng, NLG, h->Ls, nrhs, h->partial);
+    }
+    LAUNCH_CHECK(h);
+    reduce_final_kernel<<<1, 64, 0, h->stream>>>(h->partial, (int)blocks, nrhs, dev_out, ostride, ncomp);
+    LAUNCH_CHECK(h);
+    return DWF_OK;
+}
+
+extern "C" int dwf_axpy(dwf_handle h, const double* a_host, const void* x, void* y, int nrhs, int half) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS || !a_host) FAIL(h, DWF_EINVAL, "bad nrhs or a_host");
+    if (int rc = check_field(h, x, "x")) return rc;
+    if (int rc = check_field(h, y, "y")) return rc;
+    RhsCoef a;
+    for (int r = 0; r < nrhs; r++) { a.re[r] = a_host[2 * r]; a.im[r] = a_host[2 * r + 1]; }
+    const long long ng = half_groups(h, nrhs) * (half ? 1 : 2);
+    const int NLG = nrhs * h->Ls / vl(h);
+    const unsigned blocks = blas_blocks(h, ng, NLG);
+    if (h->prec == DWF_F32) axpy_kernel<float><<<blocks, 256, 0, h->stream>>>((const float4*)x, (float4*)y, ng, NLG, h->Ls, a);
+    else                    axpy_kernel<double><<<blocks, 256, 0, h->stream>>>((const double2*)x, (double2*)y, ng, NLG, h->Ls, a);
+    LAUNCH_CHECK(h);
+    return DWF_OK;
+}
+
+extern "C" int dwf_inner(dwf_handle h, const void* x, const void* y, double* out_host, int nrhs, int half) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS || !out_host) FAIL(h, DWF_EINVAL, "bad nrhs or out_host");
+    if (int rc = check_field(h, x, "x")) return rc;
+    if (int rc = check_field(h, y, "y")) return rc;
+    if (int rc = reduce_to(h, false, x, y, nrhs, half, h->scal, 2, 2)) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, 2 * nrhs * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    memcpy(out_host, h->scal_host, 2 * nrhs * sizeof(double));
+    return DWF_OK;
+}
+
+extern "C" int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs, int half) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS || !out_host) FAIL(h, DWF_EINVAL, "bad nrhs or out_host");
+    if (int rc = check_field(h, x, "x")) return rc;
+    if (int rc = reduce_to(h, true, x, nullptr, nrhs, half, h->scal, 1, 1)) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, nrhs * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    memcpy(out_host, h->scal_host, nrhs * sizeof(double));
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Red-black CGNR driver.  Host loop that only enqueues; alpha and beta are
+// computed on the device from reduction results kept in h->scal: hist[k] = |r_k|^2 at scal[k],
+// <p_k, A p_k> = |M p_k|^2 at scal[iters+1+k].
+// ------------------------------------------------------------------------------------------------
+template <typename R>
+static int cg_t(dwf_ctx* h, const void* b, void* x, int iters) {
+    using G = typename Prec<R>::G;
+    const size_t hb = half_bytes(h, 1);
+    const long long ng = half_groups(h, 1);
+    G* r = (G*)h->ws; G* p = (G*)((char*)h->ws + hb); G* w = (G*)((char*)h->ws + 2 * hb);
+    G* q = (G*)((char*)h->ws + 3 * hb); void* tmp = (char*)h->ws + 4 * hb;
+    double* hist = h->scal; double* pAp = h->scal + iters + 1;
+    const unsigned blocks = (unsigned)std::min<long long>((ng + 255) / 256, std::min<long long>((long long)h->sm_count * 8, MAX_RED_BLOCKS));
+    cudaStream_t st = h->stream;
+    if (int rc = schur_op(h, false, x, w, tmp, 1)) return rc;
+    if (int rc = schur_op(h, true, w, q, tmp, 1)) return rc;
+    cg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, q, r, p, ng, h->partial); LAUNCH_CHECK(h);
+    reduce_final_kernel<<<1, 64, 0, st>>>(h->partial, (int)blocks, 1, hist, 1, 1); LAUNCH_CHECK(h);
+    for (int k = 0; k < iters; k++) {
+        if (int rc = schur_op(h, false, p, w, tmp, 1)) return rc;
+        if (int rc = schur_op(h, true, w, q, tmp, 1)) return rc;
+        if (int rc = reduce_to(h, true, w, nullptr, 1, 1, pAp + k, 1, 1)) return rc;
+        cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, hist + k, pAp + k, h->partial); LAUNCH_CHECK(h);
+        reduce_final_kernel<<<1, 64, 0, st>>>(h->partial, (int)blocks, 1, hist + k + 1, 1, 1); LAUNCH_CHECK(h);
+        cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, hist + k + 1, hist + k); LAUNCH_CHECK(h);
+    }
+    return DWF_OK;
+}
+
+extern "C" int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, double* hist_host) {
+    if (!h) return DWF_EINVAL;
+    if (iters < 0 || 2 * iters + 2 > SCAL_DOUBLES) FAIL(h, DWF_EINVAL, "iters out of range");
+    if (int rc = check_field(h, b_even, "b_even")) return rc;
+    if (int rc = check_field(h, x_even, "x_even")) return rc;
+    if (b_even == x_even) FAIL(h, DWF_EINVAL, "b == x");
+    if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    if (int rc = need_ws(h, 5 * half_bytes(h, 1))) return rc;
+    int rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters) : cg_t<double>(h, b_even, x_even, iters);
+    if (rc) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, (iters + 1) * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (hist_host) memcpy(hist_host, h->scal_host, (iters + 1) * sizeof(double));
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// End-to-end apply from host canonical arrays (bench.py's e2e leg): H2D, import, apply, export, D2H.
+// Workspace use: [0, F) canonical staging / native out, [F, 2F) native in / canonical out, [2F, 2F+H) Schur tmp
+// ------------------------------------------------------------------------------------------------
+extern "C" int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* out_host, int nrhs) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
+    if (!in_host || !out_host) FAIL(h, DWF_EINVAL, "NULL host pointer");
+    const int base = op & ~DWF_DAGGER;
+    const bool halfop = (base == DWF_SCHUR_EO || base == DWF_MEE || base == DWF_MOOINV);
+    if (!halfop && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    if (base == DWF_SCHUR_EO && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    const size_t hb = half_bytes(h, nrhs), fb = 2 * hb;
+    if (int rc = need_ws(h, 5 * hb)) return rc;
+    char* A = (char*)h->ws; char* B = A + fb; void* tmp = A + 2 * fb;
+    void* saved_ws = h->ws; size_t saved_n = h->ws_bytes;
+    CUDA_TRY(h, cudaMemcpyAsync(A, in_host, fb, cudaMemcpyHostToDevice, h->stream));
+    // full ops: native in = B, native out = A (canonical staging is dead after import), canonical out = B
+    // half ops: native in = B[0,hb), native out = B[hb,2hb), canonical out = A (zeroed: odd sites read 0)
+    void* nat_in = B; void* nat_out = halfop ? (void*)(B + hb) : (void*)A; void* can_out = halfop ? (void*)A : (void*)B;
+    int rc = dwf_import(h, A, nat_in, nrhs, halfop ? 0 : -1);
+    if (!rc) {
+        h->ws = tmp; h->ws_bytes = hb;                 // Schur scratch lives behind the two staging buffers
+        rc = apply_checked(h, op, nat_in, nat_out, nrhs);
+        h->ws = saved_ws; h->ws_bytes = saved_n;
+    }
+    if (rc) return rc;
+    if (halfop) CUDA_TRY(h, cudaMemsetAsync(can_out, 0, fb, h->stream));
+    rc = dwf_export(h, nat_out, can_out, nrhs, halfop ? 0 : -1);
+    if (rc) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(out_host, can_out, fb, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return DWF_OK;
+}

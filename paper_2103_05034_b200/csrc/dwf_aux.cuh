@@ -1,0 +1,252 @@
+// dwf_aux.cuh -- everything on the path that is not the stencil: layout reorder (a1), the closed-form
+// M_oo^{-1} (a5), BLAS-1 with fp64 reductions (a7) and the fused CG vector updates (a9).
+#pragma once
+#include "dwf_vec.cuh"
+
+namespace dwf {
+
+// ------------------------------------------------------------------------------------------------
+// a1. canonical <-> native reorder.  canonical spinor: complex<R> [nrhs][Ls][V4 lex][12];
+// native: group index ((site*12 + c)*NLG + lg), lane = r*Ls + s, lg = lane / VL.
+// One thread per native group; blockIdx.y = parity slot.
+// ------------------------------------------------------------------------------------------------
+template <typename R, bool IMPORT>
+__global__ void reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restrict__ canon_out,
+                                      typename Prec<R>::G* native0, typename Prec<R>::G* native1,
+                                      const int* __restrict__ lex0, const int* __restrict__ lex1,
+                                      long long V4h, long long V4, int Ls, int nrhs) {
+    using G = typename Prec<R>::G;
+    constexpr int VL = Prec<R>::VL;
+    const int NLG = nrhs * Ls / VL;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= V4h * 12 * NLG) return;
+    // c fastest so that canonical accesses of neighbouring threads are contiguous (12 complex per site)
+    const int c = (int)(gid % 12);
+    const long long t2 = gid / 12;
+    const long long site = t2 % V4h;
+    const int lg = (int)(t2 / V4h);
+    G* native = blockIdx.y ? native1 : native0;
+    const int* lex = blockIdx.y ? lex1 : lex0;
+    const long long lx = lex[site];
+    const int lane = lg * VL;
+    const int r = lane / Ls, s = lane % Ls;
+    const size_t nidx = ((size_t)site * 12 + c) * NLG + lg;
+    const size_t c0 = ((((size_t)r * Ls + s) * V4 + lx) * 12 + c) * 2;
+    const size_t sstride = (size_t)V4 * 12 * 2;          // to the next s
+    if constexpr (IMPORT) {
+        if constexpr (VL == 2) native[nidx] = make_float4(canon_in[c0], canon_in[c0 + sstride], canon_in[c0 + 1], canon_in[c0 + sstride + 1]);
+        else                   native[nidx] = make_double2(canon_in[c0], canon_in[c0 + 1]);
+    } else {
+        const G g = native[nidx];
+        if constexpr (VL == 2) { canon_out[c0] = g.x; canon_out[c0 + sstride] = g.y; canon_out[c0 + 1] = g.z; canon_out[c0 + sstride + 1] = g.w; }
+        else                   { canon_out[c0] = g.x; canon_out[c0 + 1] = g.y; }
+    }
+}
+
+// canonical gauge complex<R> [mu][V4 lex][9] -> native [parity][V4h][mu][18]; U_t on the last time
+// slice is stored with the antiperiodic sign (R3).
+template <typename R>
+__global__ void reorder_gauge_kernel(const R* __restrict__ canon, R* __restrict__ native,
+                                     const int* __restrict__ lex /*[2][V4h]*/, long long V4h, long long V4,
+                                     long long spatial /*Lx*Ly*Lz*/, int Lt) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= 2 * V4h * 4 * 9) return;
+    const int k = (int)(gid % 9);
+    const int mu = (int)((gid / 9) % 4);
+    const long long ps = gid / 36;                          // p*V4h + site
+    const long long lx = lex[ps];
+    const R sign = (mu == 3 && lx / spatial == Lt - 1) ? R(-1) : R(1);
+    const size_t ci = (((size_t)mu * V4 + lx) * 9 + k) * 2;
+    native[gid * 2] = sign * canon[ci];
+    native[gid * 2 + 1] = sign * canon[ci + 1];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a5. Exact inverse of the 4D-site-diagonal block M_oo = M_ee.  Per site, per
+// complex component, per rhs the Ls x Ls system is cyclic bidiagonal:
+//    d v_j - v_{j-1} = b_j (j >= 1),   d v_0 + m v_{Ls-1} = b_0      (j = s for the P_+ half,
+//                                                                     j = Ls-1-s for the P_- half;
+//                                                                     adjoint: halves swapped)
+// solved exactly by   w_0 = 0, w_j = k (b_j + w_{j-1});  v_0 = k (b_0 - m w_{Ls-1}) / (1 + m k^Ls);
+//                     v_j = w_j + k^j v_0,               k = 1/d = 1/(5 - M5).
+// One thread per (site, component, rhs) walks s in registers.  In place is allowed.
+// ------------------------------------------------------------------------------------------------
+template <typename R, int LS, bool DAG>
+__global__ void __launch_bounds__(128)
+mooinv_kernel(const typename Prec<R>::G* in, typename Prec<R>::G* out, long long V4h, int nrhs,
+              R kappa, R mass, R v0scale /* kappa / (1 + m kappa^Ls) */) {
+    using G = typename Prec<R>::G;
+    constexpr int VL = Prec<R>::VL;
+    constexpr int NG = LS / VL;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= V4h * 12 * nrhs) return;
+    const int r = (int)(gid % nrhs);
+    const int c = (int)((gid / nrhs) % 12);
+    const long long site = gid / (12 * nrhs);
+    const size_t base = ((size_t)site * 12 + c) * ((size_t)nrhs * NG) + (size_t)r * NG;
+    const bool down = DAG ? (c >= 6) : (c < 6);
+    R bre[LS], bim[LS];
+#pragma unroll
+    for (int k = 0; k < NG; k++) {
+        const G g = in[base + (down ? k : NG - 1 - k)];
+        if constexpr (VL == 2) {
+            bre[2 * k] = down ? g.x : g.y; bre[2 * k + 1] = down ? g.y : g.x;
+            bim[2 * k] = down ? g.z : g.w; bim[2 * k + 1] = down ? g.w : g.z;
+        } else { bre[k] = g.x; bim[k] = g.y; }
+    }
+    const R b0re = bre[0], b0im = bim[0];
+    bre[0] = R(0); bim[0] = R(0);
+#pragma unroll
+    for (int j = 1; j < LS; j++) { bre[j] = kappa * (bre[j] + bre[j - 1]); bim[j] = kappa * (bim[j] + bim[j - 1]); }
+    const R v0re = v0scale * (b0re - mass * bre[LS - 1]);
+    const R v0im = v0scale * (b0im - mass * bim[LS - 1]);
+    R pw = R(1);
+#pragma unroll
+    for (int j = 0; j < LS; j++) { bre[j] = fma(pw, v0re, bre[j]); bim[j] = fma(pw, v0im, bim[j]); pw *= kappa; }
+#pragma unroll
+    for (int k = 0; k < NG; k++) {
+        G g;
+        if constexpr (VL == 2) {
+            g.x = down ? bre[2 * k] : bre[2 * k + 1]; g.y = down ? bre[2 * k + 1] : bre[2 * k];
+            g.z = down ? bim[2 * k] : bim[2 * k + 1]; g.w = down ? bim[2 * k + 1] : bim[2 * k];
+        } else { g.x = bre[k]; g.y = bim[k]; }
+        out[base + (down ? k : NG - 1 - k)] = g;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7. BLAS-1.  Fields are flat arrays of groups; group e belongs to lane group e % NLG, i.e. to rhs
+// (e % NLG) * VL / Ls.  Launch geometry guarantees (gridDim.x * blockDim.x) % NLG == 0, so a thread
+// keeps one rhs for its whole grid-stride loop.  Reductions: fp64 per-thread accumulation, fixed-
+// order in-block combine per rhs, per-block partials, fixed-order final pass => deterministic.
+// ------------------------------------------------------------------------------------------------
+struct RhsCoef { double re[64]; double im[64]; };
+
+template <typename R>
+__global__ void axpy_kernel(const typename Prec<R>::G* __restrict__ x, typename Prec<R>::G* y,
+                            long long ngroups, int NLG, int Ls, RhsCoef a) {
+    using V = typename Prec<R>::V;
+    constexpr int VL = Prec<R>::VL;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)(e % NLG) * VL / Ls;
+    const R are = (R)a.re[r], aim = (R)a.im[r];
+    for (; e < ngroups; e += stride) {
+        const CV<V> xx = unpack(ldg_nc(x + e));
+        CV<V> yy = unpack(y[e]);
+        yy.re = vfnma(aim, xx.im, vfma(are, xx.re, yy.re));
+        yy.im = vfma(aim, xx.re, vfma(are, xx.im, yy.im));
+        y[e] = pack(yy);
+    }
+}
+
+__device__ __forceinline__ void acc_inner(double& sre, double& sim, CV<float2> x, CV<float2> y) {
+    sre += (double)x.re.x * y.re.x + (double)x.im.x * y.im.x + (double)x.re.y * y.re.y + (double)x.im.y * y.im.y;
+    sim += (double)x.re.x * y.im.x - (double)x.im.x * y.re.x + (double)x.re.y * y.im.y - (double)x.im.y * y.re.y;
+}
+__device__ __forceinline__ void acc_inner(double& sre, double& sim, CV<double> x, CV<double> y) {
+    sre += x.re * y.re + x.im * y.im;
+    sim += x.re * y.im - x.im * y.re;
+}
+
+// Fixed-order combine of the 256 per-thread sums of a block into per-rhs block partials:
+// partial[(blockIdx.x * nrhs + r) * 2 + {0,1}].
+__device__ __forceinline__ void block_combine(double sre, double sim, int r, int nrhs, double* partial) {
+    __shared__ double s_re[256], s_im[256];
+    __shared__ int s_r[256];
+    s_re[threadIdx.x] = sre; s_im[threadIdx.x] = sim; s_r[threadIdx.x] = r;
+    __syncthreads();
+    if ((int)threadIdx.x < nrhs) {
+        double a = 0, b = 0;
+        for (int t = 0; t < (int)blockDim.x; t++) if (s_r[t] == (int)threadIdx.x) { a += s_re[t]; b += s_im[t]; }
+        partial[((size_t)blockIdx.x * nrhs + threadIdx.x) * 2] = a;
+        partial[((size_t)blockIdx.x * nrhs + threadIdx.x) * 2 + 1] = b;
+    }
+}
+
+template <typename R, bool NORM>
+__global__ void __launch_bounds__(256)
+inner_kernel(const typename Prec<R>::G* __restrict__ x, const typename Prec<R>::G* __restrict__ y,
+             long long ngroups, int NLG, int Ls, int nrhs, double* partial) {
+    using V = typename Prec<R>::V;
+    constexpr int VL = Prec<R>::VL;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int r = (int)(e % NLG) * VL / Ls;
+    double sre = 0, sim = 0;
+    for (; e < ngroups; e += stride) {
+        const CV<V> xx = unpack(ldg_nc(x + e));
+        if constexpr (NORM) acc_inner(sre, sim, xx, xx);
+        else                acc_inner(sre, sim, xx, unpack(ldg_nc(y + e)));
+    }
+    block_combine(sre, sim, r, nrhs, partial);
+}
+
+// out[r*ostride + {0,1}] = sum over blocks of partial, in block order.
+__global__ void reduce_final_kernel(const double* __restrict__ partial, int nblocks, int nrhs,
+                                    double* out, int ostride, int ncomp) {
+    const int r = threadIdx.x;
+    if (r >= nrhs) return;
+    double a = 0, b = 0;
+    for (int k = 0; k < nblocks; k++) { a += partial[((size_t)k * nrhs + r) * 2]; b += partial[((size_t)k * nrhs + r) * 2 + 1]; }
+    out[r * ostride] = a;
+    if (ncomp > 1) out[r * ostride + 1] = b;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a9. CG vector updates (nrhs = 1, half fields), scalars read from device memory:
+//   init  : r = b - q ; p = r ;                              partial |r|^2
+//   xr    : alpha = rr[0] / pAp[0] ; x += alpha p ; r -= alpha q ; partial |r|^2
+//   p     : beta  = rr_new[0] / rr_old[0] ; p = r + beta p
+// ------------------------------------------------------------------------------------------------
+template <typename R>
+__global__ void __launch_bounds__(256)
+cg_init_kernel(const typename Prec<R>::G* __restrict__ b, const typename Prec<R>::G* __restrict__ q,
+               typename Prec<R>::G* r, typename Prec<R>::G* p, long long ngroups, double* partial) {
+    using V = typename Prec<R>::V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double sre = 0, sim = 0;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        const CV<V> rr = csub(unpack(ldg_nc(b + e)), unpack(ldg_nc(q + e)));
+        r[e] = pack(rr); p[e] = pack(rr);
+        acc_inner(sre, sim, rr, rr);
+    }
+    block_combine(sre, sim, 0, 1, partial);
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256)
+cg_update_xr_kernel(typename Prec<R>::G* x, typename Prec<R>::G* r, const typename Prec<R>::G* __restrict__ p,
+                    const typename Prec<R>::G* __restrict__ q, long long ngroups,
+                    const double* __restrict__ rr, const double* __restrict__ pAp, double* partial) {
+    using V = typename Prec<R>::V;
+    const R alpha = (R)(rr[0] / pAp[0]);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double sre = 0, sim = 0;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        const CV<V> pp = unpack(ldg_nc(p + e)), qq = unpack(ldg_nc(q + e));
+        CV<V> xx = unpack(x[e]), rv = unpack(r[e]);
+        xx.re = vfma(alpha, pp.re, xx.re); xx.im = vfma(alpha, pp.im, xx.im);
+        rv.re = vfnma(alpha, qq.re, rv.re); rv.im = vfnma(alpha, qq.im, rv.im);
+        x[e] = pack(xx); r[e] = pack(rv);
+        acc_inner(sre, sim, rv, rv);
+    }
+    block_combine(sre, sim, 0, 1, partial);
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256)
+cg_update_p_kernel(typename Prec<R>::G* p, const typename Prec<R>::G* __restrict__ r, long long ngroups,
+                   const double* __restrict__ rr_new, const double* __restrict__ rr_old) {
+    using V = typename Prec<R>::V;
+    const R beta = (R)(rr_new[0] / rr_old[0]);
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        const CV<V> rv = unpack(ldg_nc(r + e));
+        CV<V> pp = unpack(p[e]);
+        pp.re = vfma(beta, pp.re, rv.re); pp.im = vfma(beta, pp.im, rv.im);
+        p[e] = pack(pp);
+    }
+}
+
+}  // namespace dwf

@@ -1,0 +1,208 @@
+"""ctypes binding of libdwf.so (include/dwf.h).  Same names as the C ABI, marshalling only.
+
+torch is used for device memory and streams: every field is a torch CUDA tensor whose data_ptr()
+is handed to the library.  Canonical arrays are complex tensors
+[nrhs][Ls][t][z][y][x][4][3] (spinor) / [4][t][z][y][x][3][3] (gauge); native fields are opaque
+real tensors allocated by `Dwf.field()`.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libdwf.so")
+
+DWF_F32, DWF_F64 = 0, 1
+DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV, DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV = range(7)
+DWF_DAGGER = 0x100
+_HALF_OPS = (DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV)
+
+_SIGNATURES = {
+    "dwf_create": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int), ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                  ctypes.c_int, ctypes.POINTER(ctypes.c_void_p)]),
+    "dwf_destroy": (ctypes.c_int, [ctypes.c_void_p]),
+    "dwf_set_stream": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "dwf_workspace_bytes": (ctypes.c_size_t, [ctypes.c_void_p, ctypes.c_int]),
+    "dwf_set_workspace": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t]),
+    "dwf_set_gauge": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "dwf_field_bytes": (ctypes.c_size_t, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
+    "dwf_import": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
+    "dwf_export": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
+    "dwf_apply": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dwf_apply_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dwf_chebyshev": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                     ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dwf_axpy": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_void_p, ctypes.c_void_p,
+                                ctypes.c_int, ctypes.c_int]),
+    "dwf_inner": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double),
+                                 ctypes.c_int, ctypes.c_int]),
+    "dwf_norm2": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int,
+                                 ctypes.c_int]),
+    "dwf_cg_schur": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
+                                    ctypes.POINTER(ctypes.c_double)]),
+    "dwf_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
+    "dwf_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
+}
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def exported_symbols():
+    """Names include/dwf.h declares (and this binding expects)."""
+    return sorted(_SIGNATURES)
+
+
+class DwfError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def load():
+    """Load libdwf.so; raise loudly if it has not been built (no fallback exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise DwfError(f"{_LIB_PATH} is missing: run `python -m paper_2103_05034_b200.build` "
+                           "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = ctypes.CDLL(_LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+class Dwf:
+    """One dwf_handle.  Methods are the C calls without the `dwf_` prefix."""
+
+    def __init__(self, L, Ls: int, M5: float, mass: float, precision: int, device="cuda:0"):
+        self._h = None
+        self.lib = load()
+        if not torch.cuda.is_available():
+            raise DwfError("no CUDA device: libdwf has no CPU path")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.L = tuple(int(v) for v in L)
+        self.Ls, self.M5, self.mass, self.precision = int(Ls), float(M5), float(mass), int(precision)
+        self.rdtype = torch.float32 if precision == DWF_F32 else torch.float64
+        self.cdtype = torch.complex64 if precision == DWF_F32 else torch.complex128
+        h = ctypes.c_void_p()
+        rc = self.lib.dwf_create((ctypes.c_int * 4)(*self.L), self.Ls, self.M5, self.mass, self.precision, ctypes.byref(h))
+        if rc != 0:
+            raise DwfError(f"dwf_create failed with code {rc}")
+        self._h = h
+        self._ws = None
+        self.set_stream(torch.cuda.current_stream(self.device))
+
+    # -- plumbing -------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc != 0:
+            raise DwfError(f"libdwf error {rc}: {self.lib.dwf_last_error(self._h).decode()}")
+
+    def close(self):
+        if self._h is not None:
+            torch.cuda.synchronize(self.device)
+            self.lib.dwf_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_stream(self, stream):
+        self._check(self.lib.dwf_set_stream(self._h, ctypes.c_void_p(stream.cuda_stream)))
+
+    def workspace_bytes(self, nrhs: int) -> int:
+        return int(self.lib.dwf_workspace_bytes(self._h, nrhs))
+
+    def set_workspace(self, nrhs: int):
+        """Allocate (torch) and register a workspace big enough for `nrhs` right-hand sides."""
+        n = self.workspace_bytes(nrhs)
+        if self._ws is None or self._ws.numel() < n:
+            self._ws = None
+            self._ws = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._check(self.lib.dwf_set_workspace(self._h, ctypes.c_void_p(self._ws.data_ptr()), self._ws.numel()))
+
+    def field_bytes(self, nrhs: int, half: bool = False) -> int:
+        return int(self.lib.dwf_field_bytes(self._h, nrhs, int(half)))
+
+    def field(self, nrhs: int, half: bool = False, zero: bool = False) -> torch.Tensor:
+        """Allocate a native field (opaque 1-D real tensor)."""
+        n = self.field_bytes(nrhs, half) // (4 if self.precision == DWF_F32 else 8)
+        return (torch.zeros if zero else torch.empty)(n, dtype=self.rdtype, device=self.device)
+
+    def canonical_shape(self, nrhs: int):
+        Lx, Ly, Lz, Lt = self.L
+        return (nrhs, self.Ls, Lt, Lz, Ly, Lx, 4, 3)
+
+    # -- C ABI ----------------------------------------------------------------------------------
+    def set_gauge(self, U: torch.Tensor):
+        Lx, Ly, Lz, Lt = self.L
+        assert U.is_cuda and U.dtype == self.cdtype and U.is_contiguous() and tuple(U.shape) == (4, Lt, Lz, Ly, Lx, 3, 3)
+        self._check(self.lib.dwf_set_gauge(self._h, ctypes.c_void_p(U.data_ptr())))
+
+    def import_(self, canonical: torch.Tensor, native: torch.Tensor = None, parity: int = -1) -> torch.Tensor:
+        nrhs = canonical.shape[0]
+        assert canonical.is_cuda and canonical.dtype == self.cdtype and canonical.is_contiguous()
+        assert tuple(canonical.shape) == self.canonical_shape(nrhs)
+        if native is None:
+            native = self.field(nrhs, half=(parity >= 0))
+        self._check(self.lib.dwf_import(self._h, ctypes.c_void_p(canonical.data_ptr()), ctypes.c_void_p(native.data_ptr()), nrhs, parity))
+        return native
+
+    def export(self, native: torch.Tensor, nrhs: int, parity: int = -1, canonical: torch.Tensor = None) -> torch.Tensor:
+        if canonical is None:
+            canonical = torch.zeros(self.canonical_shape(nrhs), dtype=self.cdtype, device=self.device)
+        assert canonical.is_contiguous() and canonical.dtype == self.cdtype
+        self._check(self.lib.dwf_export(self._h, ctypes.c_void_p(native.data_ptr()), ctypes.c_void_p(canonical.data_ptr()), nrhs, parity))
+        return canonical
+
+    def apply(self, op: int, inp: torch.Tensor, out: torch.Tensor, nrhs: int) -> torch.Tensor:
+        self._check(self.lib.dwf_apply(self._h, op, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr()), nrhs))
+        return out
+
+    def apply_host(self, op: int, in_host: torch.Tensor, out_host: torch.Tensor, nrhs: int) -> torch.Tensor:
+        assert not in_host.is_cuda and not out_host.is_cuda and in_host.is_contiguous() and out_host.is_contiguous()
+        self._check(self.lib.dwf_apply_host(self._h, op, ctypes.c_void_p(in_host.data_ptr()), ctypes.c_void_p(out_host.data_ptr()), nrhs))
+        return out_host
+
+    def chebyshev(self, order: int, lo: float, hi: float, inp: torch.Tensor, out: torch.Tensor, nrhs: int) -> torch.Tensor:
+        self._check(self.lib.dwf_chebyshev(self._h, order, lo, hi, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr()), nrhs))
+        return out
+
+    def axpy(self, a, x: torch.Tensor, y: torch.Tensor, nrhs: int, half: bool = False):
+        a = [complex(v) for v in a]
+        assert len(a) == nrhs
+        buf = (ctypes.c_double * (2 * nrhs))()
+        for r, v in enumerate(a):
+            buf[2 * r], buf[2 * r + 1] = v.real, v.imag
+        self._check(self.lib.dwf_axpy(self._h, buf, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(y.data_ptr()), nrhs, int(half)))
+        return y
+
+    def inner(self, x: torch.Tensor, y: torch.Tensor, nrhs: int, half: bool = False):
+        buf = (ctypes.c_double * (2 * nrhs))()
+        self._check(self.lib.dwf_inner(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(y.data_ptr()), buf, nrhs, int(half)))
+        return [complex(buf[2 * r], buf[2 * r + 1]) for r in range(nrhs)]
+
+    def norm2(self, x: torch.Tensor, nrhs: int, half: bool = False):
+        buf = (ctypes.c_double * nrhs)()
+        self._check(self.lib.dwf_norm2(self._h, ctypes.c_void_p(x.data_ptr()), buf, nrhs, int(half)))
+        return [float(buf[r]) for r in range(nrhs)]
+
+    def cg_schur(self, b_even: torch.Tensor, x_even: torch.Tensor, iters: int):
+        hist = (ctypes.c_double * (iters + 1))()
+        self._check(self.lib.dwf_cg_schur(self._h, ctypes.c_void_p(b_even.data_ptr()), ctypes.c_void_p(x_even.data_ptr()), iters, hist))
+        return [float(v) for v in hist]
+
+    def launch_count(self) -> int:
+        return int(self.lib.dwf_launch_count(self._h))

@@ -1,0 +1,154 @@
+"""GPU parity: libdwf (through its C ABI) against the CPU oracle, element by element on the same
+seeded inputs.  Tolerances are BASELINE.json north_star's: relative L2 <= 1e-12 (fp64), <= 1e-5 (fp32)
+per operator apply, <= 1e-4 for the fp32 order-64 Chebyshev filter; CG per DESIGN.md R19.
+"""
+import numpy as np
+import pytest
+
+import dwf_inputs as gen
+from gpu_util import M5, TOL_APPLY, TOL_CHEB, Rig, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+from paper_2103_05034_b200 import (DWF_DAGGER, DWF_DDW, DWF_DHOP, DWF_DPV, DWF_HDW, DWF_MEE, DWF_MOOINV,  # noqa: E402
+                                   DWF_SCHUR_EO)
+
+
+# ------------------------------------------------------------------ layout round trip (a1)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("L,Ls,nrhs", [((4, 4, 4, 4), 8, 1), ((6, 4, 8, 4), 4, 3)])
+def test_import_export_roundtrip(prec, L, Ls, nrhs):
+    rig = Rig(L, Ls, prec)
+    psi = rig.spinor(nrhs, 2000)
+    assert np.array_equal(rig.canonical(rig.native(psi), nrhs), psi)            # bit exact
+    for parity in (0, 1):
+        got = rig.canonical(rig.native(psi, parity), nrhs, parity)
+        assert np.array_equal(got, gen.keep_parity(psi, L, parity))
+
+
+# ------------------------------------------------------------------ configs[0]: 4^4 x 8
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("unit", [False, True])
+def test_config0_operators(oracle, prec, unit):
+    L, Ls, mass = (4, 4, 4, 4), 8, 0.01
+    rig = Rig(L, Ls, prec, mass, seed_U=1000, unit_links=unit)
+    psi = rig.spinor(1, 2000)
+    tol = TOL_APPLY[prec]
+    assert rel_l2(rig.apply(DWF_DHOP, psi), oracle.dhop(rig.U, psi)) < tol
+    assert rel_l2(rig.apply(DWF_DDW, psi), oracle.ddw(rig.U, psi, M5, mass)) < tol
+    assert rel_l2(rig.apply(DWF_HDW, psi), oracle.hdw(rig.U, psi, M5, mass)) < tol
+    assert rel_l2(rig.apply(DWF_DPV, psi), oracle.dpv(rig.U, psi, M5)) < tol
+    assert rel_l2(rig.apply(DWF_DHOP | DWF_DAGGER, psi), oracle.dhop(rig.U, psi, dagger=True)) < tol
+    assert rel_l2(rig.apply(DWF_DDW | DWF_DAGGER, psi), oracle.ddw(rig.U, psi, M5, mass, dagger=True)) < tol
+    assert rel_l2(rig.apply(DWF_DPV | DWF_DAGGER, psi), oracle.dpv(rig.U, psi, M5, dagger=True)) < tol
+    assert rel_l2(rig.apply(DWF_HDW | DWF_DAGGER, psi), oracle.hdw(rig.U, psi, M5, mass)) < tol
+
+
+def test_config0_point_source_golden(oracle):
+    """The hand-derived worked example (tests/golden/point_source_ddw.txt) straight on the GPU path."""
+    from test_oracle_pins import _read_golden
+    L, Ls = (4, 4, 4, 4), 8
+    rig = Rig(L, Ls, "f64", 0.01, unit_links=True)
+    out = rig.apply(DWF_DDW, gen.point_source(L, Ls, (0, 0, 0, 0), 0, 0, 0))[0]
+    expect = np.zeros_like(out)
+    for src, s, (x, y, z, t), spin, val in _read_golden():
+        if src == "A":
+            expect[s, t, z, y, x, spin, 0] = val
+    assert np.max(np.abs(out - expect)) < 1e-14
+
+
+# ------------------------------------------------------------------ ragged shapes, several rhs, all Ls
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("L,Ls,nrhs", [((6, 4, 8, 4), 4, 3), ((4, 8, 4, 6), 12, 2), ((8, 4, 4, 4), 24, 1),
+                                       ((4, 4, 4, 8), 32, 1), ((4, 4, 6, 4), 6, 5)])
+def test_ragged_shapes(oracle, prec, L, Ls, nrhs):
+    mass = 0.05
+    rig = Rig(L, Ls, prec, mass, seed_U=17)
+    psi = rig.spinor(nrhs, 18)
+    tol = TOL_APPLY[prec]
+    assert rel_l2(rig.apply(DWF_DDW, psi), oracle.ddw(rig.U, psi, M5, mass)) < tol
+    assert rel_l2(rig.apply(DWF_HDW, psi), oracle.hdw(rig.U, psi, M5, mass)) < tol
+    assert rel_l2(rig.apply(DWF_DDW | DWF_DAGGER, psi), oracle.ddw(rig.U, psi, M5, mass, dagger=True)) < tol
+    pe = gen.keep_parity(psi, L, 0)
+    assert rel_l2(rig.apply(DWF_MEE, pe, half=True), oracle.mpp(pe, M5, mass, 0)) < tol
+    assert rel_l2(rig.apply(DWF_MEE | DWF_DAGGER, pe, half=True), oracle.mpp(pe, M5, mass, 0, dagger=True)) < tol
+    if Ls in (4, 8, 12, 16, 24, 32):
+        rig.d.set_workspace(nrhs)
+        assert rel_l2(rig.apply(DWF_MOOINV, pe, half=True), oracle.mpp_inv(pe, M5, mass, 0)) < tol
+        assert rel_l2(rig.apply(DWF_MOOINV | DWF_DAGGER, pe, half=True), oracle.mpp_inv(pe, M5, mass, 0, dagger=True)) < tol
+        assert rel_l2(rig.apply(DWF_SCHUR_EO, pe, half=True), oracle.mpc(rig.U, pe, M5, mass)) < tol
+        assert rel_l2(rig.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True), oracle.mpc(rig.U, pe, M5, mass, dagger=True)) < tol
+
+
+# ------------------------------------------------------------------ configs[1]: 8^4 x 16, Schur on 4 RHS + 50 CG iterations
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_config1_schur_and_cg(oracle, prec):
+    L, Ls, mass = (8, 8, 8, 8), 16, 0.01
+    rig = Rig(L, Ls, prec, mass, seed_U=1001, ws_nrhs=4)
+    psi = gen.keep_parity(rig.spinor(4, 2001), L, 0)
+    assert rel_l2(rig.apply(DWF_SCHUR_EO, psi, half=True), oracle.mpc(rig.U, psi, M5, mass)) < TOL_APPLY[prec]
+    # CG: rhs = vector 0, x0 = 0, 50 iterations (R19 tolerances)
+    b = psi[0:1]
+    x_or, h_or = oracle.cg_schur(rig.U, b, M5, mass, 50)
+    bn = rig.native(b, 0)
+    xn = rig.d.field(1, half=True, zero=True)
+    hist = np.array(rig.d.cg_schur(bn, xn, 50))
+    x = rig.canonical(xn, 1, 0)
+    tol_h, tol_x = (1e-9, 1e-10) if prec == "f64" else (1e-4, 1e-5)
+    assert np.max(np.abs(hist - h_or) / h_or) < tol_h
+    assert rel_l2(x, x_or) < tol_x
+    assert hist[50] < 1e-4 * hist[0]                                   # it does converge
+
+
+# ------------------------------------------------------------------ BLAS-1 (a7)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("nrhs,half", [(1, False), (3, False), (4, True)])
+def test_blas1(oracle, prec, nrhs, half):
+    L, Ls = (4, 6, 4, 8), 8
+    rig = Rig(L, Ls, prec)
+    x, y = rig.spinor(nrhs, 5), rig.spinor(nrhs, 6)
+    parity = 0 if half else -1
+    if half:
+        x, y = gen.keep_parity(x, L, 0), gen.keep_parity(y, L, 0)
+    xn, yn = rig.native(x, parity), rig.native(y, parity)
+    got = np.array(rig.d.inner(xn, yn, nrhs, half))
+    want = oracle.inner(x, y)
+    assert np.max(np.abs(got - want) / np.abs(want)) < 1e-13          # fp64 accumulation on both sides
+    got = np.array(rig.d.norm2(xn, nrhs, half))
+    assert np.max(np.abs(got - oracle.norm2(x)) / oracle.norm2(x)) < 1e-13
+    a = [complex(0.3 * (r + 1), -1.1 + 0.2 * r) for r in range(nrhs)]
+    rig.d.axpy(a, xn, yn, nrhs, half)
+    assert rel_l2(rig.canonical(yn, nrhs, parity), oracle.axpy(a, x, y)) < (1e-15 if prec == "f64" else 2e-7)
+
+
+# ------------------------------------------------------------------ Chebyshev driver (a8)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("order", [0, 1, 2, 3, 64])
+def test_chebyshev_small(oracle, prec, order):
+    L, Ls, mass, nrhs = (4, 4, 4, 8), 8, 0.01, 3
+    rig = Rig(L, Ls, prec, mass, seed_U=1000, ws_nrhs=nrhs)
+    psi = rig.spinor(nrhs, 2003)
+    xn = rig.native(psi)
+    out = rig.d.field(nrhs)
+    rig.d.chebyshev(order, 0.01, 70.0, xn, out, nrhs)
+    want = oracle.chebyshev(rig.U, psi, M5, mass, order, 0.01, 70.0)
+    assert rel_l2(rig.canonical(out, nrhs), want) < TOL_CHEB[prec]
+    assert np.array_equal(rig.canonical(xn, nrhs), psi)               # input untouched
+
+
+# ------------------------------------------------------------------ error behaviour of the ABI
+def test_abi_errors():
+    from paper_2103_05034_b200 import Dwf, DwfError, DWF_F64
+    with pytest.raises(DwfError):
+        Dwf((4, 4, 4, 5), 8, M5, 0.01, DWF_F64)                        # odd extent
+    with pytest.raises(DwfError):
+        Dwf((4, 4, 4, 4), 8, 5.0, 0.01, DWF_F64)                       # M5 = 5: M_oo singular
+    d = Dwf((4, 4, 4, 4), 8, M5, 0.01, DWF_F64)
+    x, y = d.field(1), d.field(1)
+    with pytest.raises(DwfError, match="set_gauge"):
+        d.apply(DWF_DDW, x, y, 1)                                      # DWF_ENOGAUGE
+    with pytest.raises(DwfError, match="in == out"):
+        d.apply(DWF_MEE, x, x, 1)
+    d2 = Dwf((4, 4, 4, 4), 10, M5, 0.01, DWF_F64)
+    with pytest.raises(DwfError, match="instantiated"):
+        d2.apply(DWF_MOOINV, d2.field(1, half=True), d2.field(1, half=True), 1)   # Ls = 10 unsupported
