@@ -138,6 +138,49 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def run_only(args, dev):
+    """Time a single part of the step (used for ncu captures and kernel tuning)."""
+    import torch
+
+    import dwf_inputs as gen
+    from paper_2103_05034_b200 import DWF_DDW, DWF_DHOP, DWF_F32, DWF_F64, DWF_HDW, DWF_SCHUR_EO, Dwf
+    f32 = args.prec == "f32"
+    d = Dwf(L, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)
+    d.set_gauge(torch.from_numpy(gen.gauge_random(L, 1002)).to(d.cdtype).to(dev))
+    g = torch.Generator(device=dev); g.manual_seed(2002)
+    name = args.only
+    nrhs = int(name.split("nrhs")[1]) if "nrhs" in name else (CHEB_NVEC if name == "chebyshev" else 1)
+    d.set_workspace(nrhs)
+    half = name.startswith("schur") or name == "cg"
+    nb = 4 if nrhs == 1 else 1
+    xs = [d.field(nrhs, half=half).normal_(generator=g) for _ in range(nb)]
+    ys = [d.field(nrhs, half=half) for _ in range(nb)]
+    ops = {"dhop": DWF_DHOP, "ddw": DWF_DDW, "hdw": DWF_HDW, "schur": DWF_SCHUR_EO}
+
+    def once(j):
+        if name == "chebyshev":
+            d.chebyshev(CHEB_ORDER, CHEB_LO, CHEB_HI, xs[0], ys[0], nrhs)
+        elif name == "cg":
+            ys[0].zero_(); d.cg_schur(xs[0], ys[0], CG_ITERS)
+        else:
+            d.apply(ops[name.split("_")[0]], xs[j % nb], ys[j % nb], nrhs)
+    for j in range(max(args.warmup, 3)):
+        once(j)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for j in range(args.steps):
+        once(j)
+    b.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / args.steps
+    out = {"only": name, "prec": args.prec, "nrhs": nrhs, "ms": round(ms, 4)}
+    if name.split("_")[0] in ("dhop", "ddw", "hdw"):
+        by = apply_bytes(nrhs, 4 if f32 else 8)
+        out.update({"GB/s": round(by / ms / 1e6, 1), "GFlop/s": round(FLOP_PER_SITE * V5 * nrhs / ms / 1e6, 1),
+                    "frac_of_hbm_peak": round(by / ms / 1e6 / peaks()[0], 4)})
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -145,6 +188,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="dwf", choices=["dwf", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--only", default=None, help="time one part of the step only (for ncu captures), e.g. ddw_nrhs1, "
+                    "hdw_nrhs1, dhop_nrhs1, ddw_nrhs12, ddw_nrhs48, schur_nrhs4, chebyshev, cg; prints a small JSON line")
+    ap.add_argument("--prec", default="f32", choices=["f32", "f64"], help="--only mode: precision")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -163,6 +209,8 @@ def main():
     dev = torch.device(f"cuda:{local}")
     torch.cuda.set_device(dev)
     warmup = max(args.warmup, 3)
+    if args.only:
+        return run_only(args, dev)
 
     # ---- inputs (seeded, synthetic): SU(3) links from dwf_inputs (host), spinors iid N(0,1)
     # drawn directly in the native layout by torch's seeded CUDA generator (a permutation of iid Gaussians).

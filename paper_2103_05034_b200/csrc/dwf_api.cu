@@ -31,6 +31,7 @@ struct dwf_ctx {
     double* scal;         // device scalars (reduction results, CG history)
     double* scal_host;    // pinned mirror
     int sm_count;
+    long long blk_sites;  // sites per parity in one lattice block of the native site order
     long long launches;
     char err[256];
 };
@@ -53,13 +54,14 @@ static inline size_t half_bytes(const dwf_ctx* h, int nrhs) {
 static inline long long half_groups(const dwf_ctx* h, int nrhs) {
     return h->V4h * 12 * ((long long)nrhs * h->Ls / vl(h));
 }
+static inline int block_groups(const dwf_ctx* h) { return 12 * h->Ls / vl(h); }   // groups per (site, rhs) block
 
 // ------------------------------------------------------------------------------------------------
 // Index tables.  Native site order within a parity: 4D blocks of BLK^4 sites in lexicographic block
 // order, lexicographic inside a block (locality for L1/L2: DESIGN.md sec. 4.1); tables make the order
 // a free choice.  DWF_BLOCK="bx,by,bz,bt" overrides the default.
 // ------------------------------------------------------------------------------------------------
-static void build_tables(const dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nbr) {
+static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nbr) {
     const int* L = h->L;
     int B[4] = {4, 4, 4, 4};
     if (const char* env = getenv("DWF_BLOCK")) {
@@ -69,6 +71,7 @@ static void build_tables(const dwf_ctx* h, std::vector<int>& lex, std::vector<in
     for (int i = 0; i < 4; i++) if (B[i] < 1 || L[i] % B[i] != 0) B[i] = L[i];   // fall back to no blocking
     if ((B[0] * B[1] * B[2] * B[3]) % 2 != 0) B[0] = L[0];                      // blocks must hold both parities equally
     const long long V4 = h->V4, V4h = h->V4h;
+    h->blk_sites = (long long)B[0] * B[1] * B[2] * B[3] / 2;
     lex.assign(2 * V4h, 0);
     std::vector<int> idx_of(V4);                                                // lex site -> index within its parity
     long long cnt[2] = {0, 0};
@@ -238,22 +241,33 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
         a.nbr[s] = h->nbr + (size_t)p * h->V4h * 8;
         a.gauge[s] = (const R*)h->gauge + (size_t)s * h->V4h * 72;      // gauge[] is indexed by PARITY
     }
-    a.V4h = h->V4h; a.Ls = h->Ls; a.nrhs = k.nrhs; a.NLG = k.nrhs * h->Ls / Prec<R>::VL;
-    a.parity0 = k.parity0;
+    a.V4h = h->V4h; a.Ls = h->Ls; a.nrhs = k.nrhs;
+    a.parity0 = k.parity0; a.nslots = k.nslots;
+    a.chunk_blocks = h->blk_sites * k.nrhs;
     a.c_hop = (R)k.c_hop; a.c_diag = (R)(5.0 - h->M5); a.mass = (R)k.mass;
     a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c;
-    const long long threads = h->V4h * a.NLG;
-    dim3 grid((unsigned)((threads + 127) / 128), k.nslots);
+    const int K = h->Ls / Prec<R>::VL;
+    const long long nblk = h->V4h * k.nrhs;                                  // (site, rhs) blocks per parity
+    long long threads = nblk * K;
+    if (k.nslots == 2) threads = 2 * ((nblk + a.chunk_blocks - 1) / a.chunk_blocks) * a.chunk_blocks * K;
+    dim3 grid((unsigned)((threads + 127) / 128));
     cudaStream_t st = h->stream;
-#define HOPK(DAG, HOP, SELF, G5, AX) hop_kernel<R, DAG, HOP, SELF, G5, AX><<<grid, 128, 0, st>>>(a)
-    switch (k.mode) {
-        case HM_HOP:               if (k.dag) HOPK(true, true, false, false, false); else HOPK(false, true, false, false, false); break;
-        case HM_HOP_SELF:          if (k.dag) HOPK(true, true, true, false, false);  else HOPK(false, true, true, false, false); break;
-        case HM_HOP_SELF_G5:       HOPK(false, true, true, true, false); break;
-        case HM_HOP_SELF_G5_AXPBY: HOPK(false, true, true, true, true); break;
-        case HM_SELF:              if (k.dag) HOPK(true, false, true, false, false); else HOPK(false, false, true, false, false); break;
-        default: FAIL(h, DWF_EINVAL, "bad hop mode");
+#define HOPK(LS, DAG, HOP, SELF, G5, AX) hop_kernel<R, LS, DAG, HOP, SELF, G5, AX><<<grid, 128, 0, st>>>(a)
+#define HOPM(LS) \
+    switch (k.mode) { \
+        case HM_HOP:               if (k.dag) HOPK(LS, true, true, false, false, false); else HOPK(LS, false, true, false, false, false); break; \
+        case HM_HOP_SELF:          if (k.dag) HOPK(LS, true, true, true, false, false);  else HOPK(LS, false, true, true, false, false); break; \
+        case HM_HOP_SELF_G5:       HOPK(LS, false, true, true, true, false); break; \
+        case HM_HOP_SELF_G5_AXPBY: HOPK(LS, false, true, true, true, true); break; \
+        case HM_SELF:              if (k.dag) HOPK(LS, true, false, true, false, false); else HOPK(LS, false, false, true, false, false); break; \
+        default: FAIL(h, DWF_EINVAL, "bad hop mode"); \
     }
+    switch (h->Ls) {                     // compile-time Ls for the production sizes, runtime Ls otherwise
+        case 16: HOPM(16); break;
+        case 24: HOPM(24); break;
+        default: HOPM(0); break;
+    }
+#undef HOPM
 #undef HOPK
     LAUNCH_CHECK(h);
     return DWF_OK;
@@ -388,9 +402,9 @@ extern "C" int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, cons
 // ------------------------------------------------------------------------------------------------
 // BLAS-1
 // ------------------------------------------------------------------------------------------------
-static unsigned blas_blocks(const dwf_ctx* h, long long ngroups, int NLG) {
-    // (blocks * 256) % NLG == 0 so that each thread keeps one rhs over its grid-stride loop
-    const long long unit = NLG / std::gcd((long long)NLG, 256LL);
+static unsigned blas_blocks(const dwf_ctx* h, long long ngroups, long long period) {
+    // (blocks * 256) % period == 0 (period = groups per site = BS * nrhs) so that each thread keeps one rhs
+    const long long unit = period / std::gcd(period, 256LL);
     long long want = std::min<long long>((ngroups + 255) / 256, (long long)h->sm_count * 8);
     long long blocks = std::max<long long>(unit, (want / unit) * unit);
     if (blocks > MAX_RED_BLOCKS) blocks = std::max<long long>(unit, (MAX_RED_BLOCKS / unit) * unit);
@@ -399,14 +413,14 @@ static unsigned blas_blocks(const dwf_ctx* h, long long ngroups, int NLG) {
 
 static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp) {
     const long long ng = half_groups(h, nrhs) * (half ? 1 : 2);
-    const int NLG = nrhs * h->Ls / vl(h);
-    const unsigned blocks = blas_blocks(h, ng, NLG);
+    const int BS = block_groups(h);
+    const unsigned blocks = blas_blocks(h, ng, (long long)BS * nrhs);
     if (h->prec == DWF_F32) {
-        if (norm) inner_kernel<float, true><<<blocks, 256, 0, h->stream>>>((const float4*)x, nullptr, ng, NLG, h->Ls, nrhs, h->partial);
-        else      inner_kernel<float, false><<<blocks, 256, 0, h->stream>>>((const float4*)x, (const float4*)y, ng, NLG, h->Ls, nrhs, h->partial);
+        if (norm) inner_kernel<float, true><<<blocks, 256, 0, h->stream>>>((const float4*)x, nullptr, ng, BS, nrhs, h->partial);
+        else      inner_kernel<float, false><<<blocks, 256, 0, h->stream>>>((const float4*)x, (const float4*)y, ng, BS, nrhs, h->partial);
     } else {
-        if (norm) inner_kernel<double, true><<<blocks, 256, 0, h->stream>>>((const double2*)x, nullptr, ng, NLG, h->Ls, nrhs, h->partial);
-        else      inner_kernel<double, false><<<blocks, 256, 0, h->stream>>>((const double2*)x, (const double2*)y, ng, NLG, h->Ls, nrhs, h->partial);
+        if (norm) inner_kernel<double, true><<<blocks, 256, 0, h->stream>>>((const double2*)x, nullptr, ng, BS, nrhs, h->partial);
+        else      inner_kernel<double, false><<<blocks, 256, 0, h->stream>>>((const double2*)x, (const double2*)y, ng, BS, nrhs, h->partial);
     }
     LAUNCH_CHECK(h);
     reduce_final_kernel<<<1, 64, 0, h->stream>>>(h->partial, (int)blocks, nrhs, dev_out, ostride, ncomp);
@@ -422,10 +436,10 @@ extern "C" int dwf_axpy(dwf_handle h, const double* a_host, const void* x, void*
     RhsCoef a;
     for (int r = 0; r < nrhs; r++) { a.re[r] = a_host[2 * r]; a.im[r] = a_host[2 * r + 1]; }
     const long long ng = half_groups(h, nrhs) * (half ? 1 : 2);
-    const int NLG = nrhs * h->Ls / vl(h);
-    const unsigned blocks = blas_blocks(h, ng, NLG);
-    if (h->prec == DWF_F32) axpy_kernel<float><<<blocks, 256, 0, h->stream>>>((const float4*)x, (float4*)y, ng, NLG, h->Ls, a);
-    else                    axpy_kernel<double><<<blocks, 256, 0, h->stream>>>((const double2*)x, (double2*)y, ng, NLG, h->Ls, a);
+    const int BS = block_groups(h);
+    const unsigned blocks = blas_blocks(h, ng, (long long)BS * nrhs);
+    if (h->prec == DWF_F32) axpy_kernel<float><<<blocks, 256, 0, h->stream>>>((const float4*)x, (float4*)y, ng, BS, nrhs, a);
+    else                    axpy_kernel<double><<<blocks, 256, 0, h->stream>>>((const double2*)x, (double2*)y, ng, BS, nrhs, a);
     LAUNCH_CHECK(h);
     return DWF_OK;
 }

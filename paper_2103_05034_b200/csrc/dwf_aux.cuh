@@ -7,7 +7,7 @@ namespace dwf {
 
 // ------------------------------------------------------------------------------------------------
 // a1. canonical <-> native reorder.  canonical spinor: complex<R> [nrhs][Ls][V4 lex][12];
-// native: group index ((site*12 + c)*NLG + lg), lane = r*Ls + s, lg = lane / VL.
+// native: group index (((site*nrhs + r)*12 + c)*K + k), K = Ls/VL, group k holds lanes s = k*VL .. k*VL+VL-1.
 // One thread per native group; blockIdx.y = parity slot.
 // ------------------------------------------------------------------------------------------------
 template <typename R, bool IMPORT>
@@ -17,9 +17,9 @@ __global__ void reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restr
                                       long long V4h, long long V4, int Ls, int nrhs) {
     using G = typename Prec<R>::G;
     constexpr int VL = Prec<R>::VL;
-    const int NLG = nrhs * Ls / VL;
+    const int K = Ls / VL;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= V4h * 12 * NLG) return;
+    if (gid >= V4h * 12 * nrhs * K) return;
     // c fastest so that canonical accesses of neighbouring threads are contiguous (12 complex per site)
     const int c = (int)(gid % 12);
     const long long t2 = gid / 12;
@@ -28,9 +28,8 @@ __global__ void reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restr
     G* native = blockIdx.y ? native1 : native0;
     const int* lex = blockIdx.y ? lex1 : lex0;
     const long long lx = lex[site];
-    const int lane = lg * VL;
-    const int r = lane / Ls, s = lane % Ls;
-    const size_t nidx = ((size_t)site * 12 + c) * NLG + lg;
+    const int r = lg / K, k = lg % K, s = k * VL;
+    const size_t nidx = (((size_t)site * nrhs + r) * 12 + c) * K + k;
     const size_t c0 = ((((size_t)r * Ls + s) * V4 + lx) * 12 + c) * 2;
     const size_t sstride = (size_t)V4 * 12 * 2;          // to the next s
     if constexpr (IMPORT) {
@@ -83,7 +82,7 @@ mooinv_kernel(const typename Prec<R>::G* in, typename Prec<R>::G* out, long long
     const int r = (int)(gid % nrhs);
     const int c = (int)((gid / nrhs) % 12);
     const long long site = gid / (12 * nrhs);
-    const size_t base = ((size_t)site * 12 + c) * ((size_t)nrhs * NG) + (size_t)r * NG;
+    const size_t base = (((size_t)site * nrhs + r) * 12 + c) * NG;
     const bool down = DAG ? (c >= 6) : (c < 6);
     R bre[LS], bim[LS];
 #pragma unroll
@@ -115,21 +114,20 @@ mooinv_kernel(const typename Prec<R>::G* in, typename Prec<R>::G* out, long long
 }
 
 // ------------------------------------------------------------------------------------------------
-// a7. BLAS-1.  Fields are flat arrays of groups; group e belongs to lane group e % NLG, i.e. to rhs
-// (e % NLG) * VL / Ls.  Launch geometry guarantees (gridDim.x * blockDim.x) % NLG == 0, so a thread
-// keeps one rhs for its whole grid-stride loop.  Reductions: fp64 per-thread accumulation, fixed-
+// a7. BLAS-1.  Fields are flat arrays of groups; group e belongs to rhs (e / BS) % nrhs, BS = 12*Ls/VL
+// groups per (site, rhs) block.  Launch geometry guarantees (gridDim.x * blockDim.x) % (BS*nrhs) == 0,
+// so a thread keeps one rhs for its whole grid-stride loop.  Reductions: fp64 per-thread accumulation, fixed-
 // order in-block combine per rhs, per-block partials, fixed-order final pass => deterministic.
 // ------------------------------------------------------------------------------------------------
 struct RhsCoef { double re[64]; double im[64]; };
 
 template <typename R>
 __global__ void axpy_kernel(const typename Prec<R>::G* __restrict__ x, typename Prec<R>::G* y,
-                            long long ngroups, int NLG, int Ls, RhsCoef a) {
+                            long long ngroups, int BS, int nrhs, RhsCoef a) {
     using V = typename Prec<R>::V;
-    constexpr int VL = Prec<R>::VL;
     const long long stride = (long long)gridDim.x * blockDim.x;
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int r = (int)(e % NLG) * VL / Ls;
+    const int r = (int)((e / BS) % nrhs);
     const R are = (R)a.re[r], aim = (R)a.im[r];
     for (; e < ngroups; e += stride) {
         const CV<V> xx = unpack(ldg_nc(x + e));
@@ -167,12 +165,11 @@ __device__ __forceinline__ void block_combine(double sre, double sim, int r, int
 template <typename R, bool NORM>
 __global__ void __launch_bounds__(256)
 inner_kernel(const typename Prec<R>::G* __restrict__ x, const typename Prec<R>::G* __restrict__ y,
-             long long ngroups, int NLG, int Ls, int nrhs, double* partial) {
+             long long ngroups, int BS, int nrhs, double* partial) {
     using V = typename Prec<R>::V;
-    constexpr int VL = Prec<R>::VL;
     const long long stride = (long long)gridDim.x * blockDim.x;
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int r = (int)(e % NLG) * VL / Ls;
+    const int r = (int)((e / BS) % nrhs);
     double sre = 0, sim = 0;
     for (; e < ngroups; e += stride) {
         const CV<V> xx = unpack(ldg_nc(x + e));

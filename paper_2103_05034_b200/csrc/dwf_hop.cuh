@@ -28,8 +28,10 @@ template <typename R> struct HopArgs {
     const R* gauge[2];     // [q] links stored at sites of parity q: [V4h][mu 4][18 reals]
     const int* nbr[2];     // [p] neighbour table of parity-p sites: [V4h][8], slot 2mu = +mu, 2mu+1 = -mu
     long long V4h;
-    int Ls, nrhs, NLG;     // NLG = nrhs * Ls / VL lane groups per site
-    int parity0;           // output parity of blockIdx.y == 0
+    int Ls, nrhs;          // runtime Ls (used when the kernel's LS template parameter is 0)
+    int parity0;           // output parity of slot 0
+    int nslots;            // 1: one output parity; 2: both, interleaved in chunks of chunk_blocks (site,rhs) blocks
+    long long chunk_blocks;
     R c_hop, c_diag, mass;
     R ax_a, ax_b, ax_c;
 };
@@ -56,7 +58,7 @@ __device__ __forceinline__ void su3_mul(const R (&u)[18], const CV<V> (&h)[3], C
 // One direction of the stencil.  MU = 0..3 (x,y,z,t); SG = -1: projector (1 - gamma_mu), +1: (1 + gamma_mu)
 // (chiral basis R1; the rank-2 forms below are the rows of the 4x4 matrices written out).
 template <int MU, int SG, bool FWD, typename R, typename V, typename G>
-__device__ __forceinline__ void hop_dir(CV<V> (&acc)[12], const G* __restrict__ psi, size_t cstride,
+__device__ __forceinline__ void hop_dir(CV<V> (&acc)[12], const G* __restrict__ psi, const int cstride,
                                         const R* __restrict__ link) {
     CV<V> p[12];
 #pragma unroll
@@ -115,29 +117,29 @@ __device__ __forceinline__ void hop_dir(CV<V> (&acc)[12], const G* __restrict__ 
 // Components c < 6 are the P_+ half (spins 0,1), c >= 6 the P_- half (R2).  Non-adjoint: P_+ couples
 // to s-1 (wall: +m psi(Ls-1) at s = 0), P_- to s+1 (wall: +m psi(0) at s = Ls-1).  Adjoint: swapped.
 //
-// fp32: this thread holds lanes (sa, sb) = (2k, 2k+1) of rhs r.
+// fp32: this thread holds lanes (sa, sb) = (2k, 2k+1) of its (site, rhs) block (K = Ls/2 groups per component).
 //   "s-1" rule: neighbours (2k-1, 2k)   = (prev group .y, own .x), coefficients (k==0 ? m : -1, -1)
 //   "s+1" rule: neighbours (2k+1, 2k+2) = (own .y, next group .x), coefficients (-1, k==last ? m : -1)
 template <bool DAG>
-__device__ __forceinline__ void self_term(CV<float2> (&res)[12], const float4* __restrict__ site_base,
-                                          size_t cstride, int lg, int Ls, float c_diag, float mass) {
-    const int half = Ls >> 1;
-    const int k = lg % half;
-    const int r0 = lg - k;                                   // first group of this rhs
-    const int kprev = (k == 0) ? half - 1 : k - 1;
-    const int knext = (k == half - 1) ? 0 : k + 1;
+__device__ __forceinline__ void self_term(CV<float2> (&res)[12], const float4* __restrict__ blk,
+                                          const int K, const int k, float c_diag, float mass) {
+    const int kprev = (k == 0) ? K - 1 : k - 1;
+    const int knext = (k == K - 1) ? 0 : k + 1;
     const float2 coef_dn = make_float2((k == 0) ? mass : -1.f, -1.f);
-    const float2 coef_up = make_float2(-1.f, (k == half - 1) ? mass : -1.f);
+    const float2 coef_up = make_float2(-1.f, (k == K - 1) ? mass : -1.f);
+    const float4* own_p = blk + k;
+    const float4* dn_p = blk + kprev;
+    const float4* up_p = blk + knext;
 #pragma unroll
     for (int c = 0; c < 12; c++) {
-        const CV<float2> own = unpack(ldg_nc(site_base + c * cstride + lg));
+        const CV<float2> own = unpack(ldg_nc(own_p + c * K));
         const bool down = DAG ? (c >= 6) : (c < 6);          // couples to s-1 ?
         CV<float2> t; float2 coef;
         if (down) {
-            const CV<float2> o = unpack(ldg_nc(site_base + c * cstride + r0 + kprev));
+            const CV<float2> o = unpack(ldg_nc(dn_p + c * K));
             t.re = make_float2(o.re.y, own.re.x); t.im = make_float2(o.im.y, own.im.x); coef = coef_dn;
         } else {
-            const CV<float2> o = unpack(ldg_nc(site_base + c * cstride + r0 + knext));
+            const CV<float2> o = unpack(ldg_nc(up_p + c * K));
             t.re = make_float2(own.re.y, o.re.x); t.im = make_float2(own.im.y, o.im.x); coef = coef_up;
         }
         res[c].re = vfma2(coef, t.re, vfma(c_diag, own.re, res[c].re));
@@ -145,46 +147,49 @@ __device__ __forceinline__ void self_term(CV<float2> (&res)[12], const float4* _
     }
 }
 
-// fp64: this thread holds lane s of rhs r.
+// fp64: this thread holds lane s = k of its (site, rhs) block (K = Ls).
 template <bool DAG>
-__device__ __forceinline__ void self_term(CV<double> (&res)[12], const double2* __restrict__ site_base,
-                                          size_t cstride, int lg, int Ls, double c_diag, double mass) {
-    const int s = lg % Ls;
-    const int r0 = lg - s;
-    const int sprev = (s == 0) ? Ls - 1 : s - 1;
-    const int snext = (s == Ls - 1) ? 0 : s + 1;
-    const double coef_dn = (s == 0) ? mass : -1.0;
-    const double coef_up = (s == Ls - 1) ? mass : -1.0;
+__device__ __forceinline__ void self_term(CV<double> (&res)[12], const double2* __restrict__ blk,
+                                          const int K, const int k, double c_diag, double mass) {
+    const int sprev = (k == 0) ? K - 1 : k - 1;
+    const int snext = (k == K - 1) ? 0 : k + 1;
+    const double coef_dn = (k == 0) ? mass : -1.0;
+    const double coef_up = (k == K - 1) ? mass : -1.0;
 #pragma unroll
     for (int c = 0; c < 12; c++) {
-        const CV<double> own = unpack(ldg_nc(site_base + c * cstride + lg));
+        const CV<double> own = unpack(ldg_nc(blk + c * K + k));
         const bool down = DAG ? (c >= 6) : (c < 6);
-        const CV<double> o = unpack(ldg_nc(site_base + c * cstride + r0 + (down ? sprev : snext)));
+        const CV<double> o = unpack(ldg_nc(blk + c * K + (down ? sprev : snext)));
         const double coef = down ? coef_dn : coef_up;
         res[c].re = fma(coef, o.re, fma(c_diag, own.re, res[c].re));
         res[c].im = fma(coef, o.im, fma(c_diag, own.im, res[c].im));
     }
 }
 
-// Gamma5 = gamma5 R5 target lane group and lane swap (eq. 6, R6)
-__device__ __forceinline__ int g5_target(int lg, int Ls, float) {
-    const int half = Ls >> 1; const int k = lg % half; return lg - k + (half - 1 - k);
-}
-__device__ __forceinline__ int g5_target(int lg, int Ls, double) {
-    const int s = lg % Ls; return lg - s + (Ls - 1 - s);
-}
-
-template <typename R, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY>
-__global__ void __launch_bounds__(128)
+// Gamma5 = gamma5 R5 (eq. 6, R6): lane group k of a block goes to group K-1-k (fp32: the two lanes
+// of the group also swap).
+template <typename R, int LS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY>
+__global__ void __launch_bounds__(128, 4)
 hop_kernel(const HopArgs<R> a) {
     using V = typename Prec<R>::V;
     using G = typename Prec<R>::G;
+    constexpr int VL = Prec<R>::VL;
+    const int K = (LS > 0) ? LS / VL : a.Ls / VL;            // lane groups per component of a (site, rhs) block
+    // ---- which (output parity slot, site, rhs, lane group) is this thread? ------------------------------
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const long long site = gid / a.NLG;
+    long long blk = gid / K;                                  // (site, rhs) block index, maybe across both slots
+    const int k = (int)(gid - blk * K);
+    int pi = 0;
+    if (a.nslots == 2) {                                      // chunks of chunk_blocks alternate between the parities
+        const long long q = blk / (2 * a.chunk_blocks);
+        const long long rem = blk - q * 2 * a.chunk_blocks;
+        pi = rem >= a.chunk_blocks;
+        blk = q * a.chunk_blocks + (rem - pi * a.chunk_blocks);
+    }
+    const long long site = blk / a.nrhs;
     if (site >= a.V4h) return;
-    const int lg = (int)(gid - site * a.NLG);
-    const int pi = blockIdx.y;                      // which output-parity slot
-    const size_t cstride = (size_t)a.NLG;
+    const int r = (int)(blk - site * a.nrhs);
+    const int BS = 12 * K;                                    // groups per block
 
     CV<V> acc[12];
 #pragma unroll
@@ -194,48 +199,49 @@ hop_kernel(const HopArgs<R> a) {
         const int p = (a.parity0 + pi) & 1;
         const int4* nb4 = reinterpret_cast<const int4*>(a.nbr[pi] + site * 8);
         const int4 n0 = __ldg(nb4), n1 = __ldg(nb4 + 1);
-        const G* in = a.in_hop[pi] + lg;
+        const G* in = a.in_hop[pi] + (size_t)r * BS + k;
+        const size_t sstride = (size_t)a.nrhs * BS;           // groups per site
         const R* u_own = a.gauge[p] + (size_t)site * 72;
         const R* u_nbr = a.gauge[p ^ 1];
-        constexpr int SF = DAG ? +1 : -1;           // projector sign on the forward hop
-        hop_dir<0, SF, true >(acc, in + (size_t)n0.x * 12 * cstride, cstride, u_own + 0);
-        hop_dir<0, -SF, false>(acc, in + (size_t)n0.y * 12 * cstride, cstride, u_nbr + (size_t)n0.y * 72 + 0);
-        hop_dir<1, SF, true >(acc, in + (size_t)n0.z * 12 * cstride, cstride, u_own + 18);
-        hop_dir<1, -SF, false>(acc, in + (size_t)n0.w * 12 * cstride, cstride, u_nbr + (size_t)n0.w * 72 + 18);
-        hop_dir<2, SF, true >(acc, in + (size_t)n1.x * 12 * cstride, cstride, u_own + 36);
-        hop_dir<2, -SF, false>(acc, in + (size_t)n1.y * 12 * cstride, cstride, u_nbr + (size_t)n1.y * 72 + 36);
-        hop_dir<3, SF, true >(acc, in + (size_t)n1.z * 12 * cstride, cstride, u_own + 54);
-        hop_dir<3, -SF, false>(acc, in + (size_t)n1.w * 12 * cstride, cstride, u_nbr + (size_t)n1.w * 72 + 54);
+        constexpr int SF = DAG ? +1 : -1;                     // projector sign on the forward hop
+        hop_dir<0, SF, true >(acc, in + (size_t)n0.x * sstride, K, u_own + 0);
+        hop_dir<0, -SF, false>(acc, in + (size_t)n0.y * sstride, K, u_nbr + (size_t)n0.y * 72 + 0);
+        hop_dir<1, SF, true >(acc, in + (size_t)n0.z * sstride, K, u_own + 18);
+        hop_dir<1, -SF, false>(acc, in + (size_t)n0.w * sstride, K, u_nbr + (size_t)n0.w * 72 + 18);
+        hop_dir<2, SF, true >(acc, in + (size_t)n1.x * sstride, K, u_own + 36);
+        hop_dir<2, -SF, false>(acc, in + (size_t)n1.y * sstride, K, u_nbr + (size_t)n1.y * 72 + 36);
+        hop_dir<3, SF, true >(acc, in + (size_t)n1.z * sstride, K, u_own + 54);
+        hop_dir<3, -SF, false>(acc, in + (size_t)n1.w * sstride, K, u_nbr + (size_t)n1.w * 72 + 54);
 #pragma unroll
         for (int c = 0; c < 12; c++) { acc[c].re = vmul(a.c_hop, acc[c].re); acc[c].im = vmul(a.c_hop, acc[c].im); }
     }
     if constexpr (SELF) {
-        self_term<DAG>(acc, a.in_self[pi] + (size_t)site * 12 * cstride, cstride, lg, a.Ls, a.c_diag, a.mass);
+        self_term<DAG>(acc, a.in_self[pi] + (size_t)blk * BS, K, k, a.c_diag, a.mass);
     }
-    int lgo = lg;
+    int ko = k;
     if constexpr (G5) {
-        lgo = g5_target(lg, a.Ls, R());
+        ko = K - 1 - k;
 #pragma unroll
         for (int c = 0; c < 12; c++) {
             acc[c].re = vswap(acc[c].re); acc[c].im = vswap(acc[c].im);
             if (c >= 6) { acc[c].re = vneg(acc[c].re); acc[c].im = vneg(acc[c].im); }
         }
     }
-    const size_t obase = (size_t)site * 12 * cstride + lgo;
+    const size_t obase = (size_t)blk * BS + ko;
     if constexpr (AXPBY) {
         const G* y = a.y[pi] + obase;
         const G* z = a.z[pi] + obase;
 #pragma unroll
         for (int c = 0; c < 12; c++) {
-            const CV<V> yy = unpack(ldg_nc(y + c * cstride));
-            const CV<V> zz = unpack(ld_plain(z + c * cstride));
+            const CV<V> yy = unpack(ldg_nc(y + c * K));
+            const CV<V> zz = unpack(ld_plain(z + c * K));
             acc[c].re = vfma(a.ax_c, zz.re, vfma(a.ax_b, yy.re, vmul(a.ax_a, acc[c].re)));
             acc[c].im = vfma(a.ax_c, zz.im, vfma(a.ax_b, yy.im, vmul(a.ax_a, acc[c].im)));
         }
     }
     G* o = a.out[pi] + obase;
 #pragma unroll
-    for (int c = 0; c < 12; c++) o[c * cstride] = pack(acc[c]);
+    for (int c = 0; c < 12; c++) o[c * K] = pack(acc[c]);
 }
 
 }  // namespace dwf
