@@ -138,6 +138,19 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def combine_over_ranks(ms: float, launches: int, dev, world: int):
+    """Replicas: the job's time is the MAX over ranks, its kernel-launch count the SUM."""
+    if world <= 1:
+        return ms, launches
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([ms], device=dev, dtype=torch.float64)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    ll = torch.tensor([launches], device=dev, dtype=torch.int64)
+    dist.all_reduce(ll)
+    return float(tt.item()), int(ll.item())
+
+
 def run_only(args, dev):
     """Time a single part of the step (used for ncu captures and kernel tuning)."""
     import torch
@@ -286,11 +299,7 @@ def main():
     clocks = sampler.stop() if sampler else None
     launches = d.launch_count() - l0
     ms = s.elapsed_time(e)
-    if world > 1:
-        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX); ms = float(tt.item())
-        ll = torch.tensor([launches], device=dev, dtype=torch.int64)
-        dist.all_reduce(ll); launches = int(ll.item())
+    ms, launches = combine_over_ranks(ms, launches, dev, world)
 
     # ---- e2e: the same apply through the C ABI with HOST buffers (H2D + D2H inside the timed region)
     for _ in range(2):
@@ -302,9 +311,7 @@ def main():
         d.apply_host(DWF_DDW, host_in, host_out, 1)
     torch.cuda.synchronize()
     e2e_s = (time.perf_counter() - t0) / ne2e
-    if world > 1:
-        tt = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX); e2e_s = float(tt.item())
+    e2e_s, _ = combine_over_ranks(e2e_s, 0, dev, world)
 
     if rank != 0:
         if world > 1:

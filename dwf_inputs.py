@@ -105,3 +105,43 @@ def point_source(L, Ls: int, site, s: int, spin: int, colour: int) -> np.ndarray
     x, y, z, t = site
     psi[0, s, t, z, y, x, spin, colour] = 1.0
     return psi
+
+
+# ---- device-side generation for lattices too big to draw on the host (configs[4]) -------------------
+def su3_from_gaussian_torch(g):
+    """Same recipe as su3_from_gaussian (R15) on a torch complex tensor [...,3,3] (any device)."""
+    import torch
+    r0 = g[..., 0, :]
+    r1 = g[..., 1, :]
+    r0 = r0 / torch.sqrt(torch.sum(r0.abs() ** 2, dim=-1, keepdim=True))
+    proj = torch.sum(torch.conj(r0) * r1, dim=-1, keepdim=True)
+    r1 = r1 - r0 * proj
+    r1 = r1 / torch.sqrt(torch.sum(r1.abs() ** 2, dim=-1, keepdim=True))
+    r2 = torch.conj(torch.linalg.cross(r0, r1))
+    return torch.stack([r0, r1, r2], dim=-2)
+
+
+def gauge_random_torch(L, seed: int, device, dtype):
+    """Random SU(3) gauge field drawn on `device` with torch's seeded generator, one direction at a time."""
+    import torch
+    Lx, Ly, Lz, Lt = (int(v) for v in L)
+    gen_ = torch.Generator(device=device); gen_.manual_seed(seed)
+    rdt = torch.float32 if dtype == torch.complex64 else torch.float64
+    U = torch.empty((4, Lt, Lz, Ly, Lx, 3, 3), dtype=dtype, device=device)
+    for mu in range(4):
+        g = torch.view_as_complex(torch.randn((Lt, Lz, Ly, Lx, 3, 3, 2), generator=gen_, device=device, dtype=rdt))
+        U[mu] = su3_from_gaussian_torch(g)
+    return U
+
+
+def spinor_gaussian_torch(L, Ls: int, nrhs: int, seed: int, device, dtype):
+    """Gaussian spinor fields drawn on `device`: canonical [nrhs][Ls][t][z][y][x][4][3]."""
+    import torch
+    Lx, Ly, Lz, Lt = (int(v) for v in L)
+    gen_ = torch.Generator(device=device); gen_.manual_seed(seed)
+    rdt = torch.float32 if dtype == torch.complex64 else torch.float64
+    out = torch.empty((nrhs, Ls, Lt, Lz, Ly, Lx, 4, 3), dtype=dtype, device=device)
+    for r in range(nrhs):
+        for s in range(Ls):
+            out[r, s] = torch.view_as_complex(torch.randn((Lt, Lz, Ly, Lx, 4, 3, 2), generator=gen_, device=device, dtype=rdt))
+    return out

@@ -32,6 +32,7 @@ struct dwf_ctx {
     double* scal_host;    // pinned mirror
     int sm_count;
     long long blk_sites;  // sites per parity in one lattice block of the native site order
+    int rhs_chunk;        // right-hand sides per stencil launch
     long long launches;
     char err[256];
 };
@@ -63,28 +64,34 @@ static inline int block_groups(const dwf_ctx* h) { return 12 * h->Ls / vl(h); } 
 // ------------------------------------------------------------------------------------------------
 static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nbr) {
     const int* L = h->L;
-    int B[4] = {4, 4, 4, 4};
-    if (const char* env = getenv("DWF_BLOCK")) {
-        int b[4];
-        if (sscanf(env, "%d,%d,%d,%d", &b[0], &b[1], &b[2], &b[3]) == 4) for (int i = 0; i < 4; i++) B[i] = b[i];
-    }
+    int B[4] = {4, 4, 4, 4};      // outer block: unit of the parity interleave, L2 locality
+    int T[4] = {4, 4, 2, 2};      // inner tile : 32 sites per parity = what one CTA works on (L1 locality)
+    auto parse = [](const char* name, int* v) {
+        if (const char* env = getenv(name)) { int b[4]; if (sscanf(env, "%d,%d,%d,%d", &b[0], &b[1], &b[2], &b[3]) == 4) for (int i = 0; i < 4; i++) v[i] = b[i]; }
+    };
+    parse("DWF_BLOCK", B); parse("DWF_TILE", T);
     for (int i = 0; i < 4; i++) if (B[i] < 1 || L[i] % B[i] != 0) B[i] = L[i];   // fall back to no blocking
     if ((B[0] * B[1] * B[2] * B[3]) % 2 != 0) B[0] = L[0];                      // blocks must hold both parities equally
+    for (int i = 0; i < 4; i++) if (T[i] < 1 || B[i] % T[i] != 0) T[i] = B[i];
+    if ((T[0] * T[1] * T[2] * T[3]) % 2 != 0) for (int i = 0; i < 4; i++) T[i] = B[i];
     const long long V4 = h->V4, V4h = h->V4h;
     h->blk_sites = (long long)B[0] * B[1] * B[2] * B[3] / 2;
     lex.assign(2 * V4h, 0);
     std::vector<int> idx_of(V4);                                                // lex site -> index within its parity
     long long cnt[2] = {0, 0};
-    int nb[4]; for (int i = 0; i < 4; i++) nb[i] = L[i] / B[i];
+    int nb[4], nt[4]; for (int i = 0; i < 4; i++) { nb[i] = L[i] / B[i]; nt[i] = B[i] / T[i]; }
     for (int bt = 0; bt < nb[3]; bt++) for (int bz = 0; bz < nb[2]; bz++) for (int by = 0; by < nb[1]; by++) for (int bx = 0; bx < nb[0]; bx++)
-        for (int t = bt * B[3]; t < (bt + 1) * B[3]; t++) for (int z = bz * B[2]; z < (bz + 1) * B[2]; z++)
-            for (int y = by * B[1]; y < (by + 1) * B[1]; y++) for (int x = bx * B[0]; x < (bx + 1) * B[0]; x++) {
+      for (int tt = 0; tt < nt[3]; tt++) for (int tz = 0; tz < nt[2]; tz++) for (int ty = 0; ty < nt[1]; ty++) for (int tx = 0; tx < nt[0]; tx++) {
+        const int o[4] = {bx * B[0] + tx * T[0], by * B[1] + ty * T[1], bz * B[2] + tz * T[2], bt * B[3] + tt * T[3]};
+        for (int t = o[3]; t < o[3] + T[3]; t++) for (int z = o[2]; z < o[2] + T[2]; z++)
+            for (int y = o[1]; y < o[1] + T[1]; y++) for (int x = o[0]; x < o[0] + T[0]; x++) {
                 const int p = (x + y + z + t) & 1;
                 const long long lx = x + (long long)L[0] * (y + (long long)L[1] * (z + (long long)L[2] * t));
                 lex[p * V4h + cnt[p]] = (int)lx;
                 idx_of[lx] = (int)cnt[p];
                 cnt[p]++;
             }
+      }
     nbr.assign(2 * V4h * 8, 0);
     for (int p = 0; p < 2; p++) for (long long i = 0; i < V4h; i++) {
         long long lx = lex[p * V4h + i];
@@ -122,6 +129,8 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
     }
     std::vector<int> lex, nbr;
     build_tables(h, lex, nbr);
+    h->rhs_chunk = 4;
+    if (const char* env = getenv("DWF_RHS_CHUNK")) h->rhs_chunk = std::max(1, atoi(env));
     const size_t gbytes = (size_t)2 * h->V4h * 72 * real_bytes(h);
     bool ok = cudaMalloc(&h->gauge, gbytes) == cudaSuccess
            && cudaMalloc((void**)&h->nbr, nbr.size() * sizeof(int)) == cudaSuccess
@@ -243,16 +252,16 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     }
     a.V4h = h->V4h; a.Ls = h->Ls; a.nrhs = k.nrhs;
     a.parity0 = k.parity0; a.nslots = k.nslots;
-    a.chunk_blocks = h->blk_sites * k.nrhs;
     a.c_hop = (R)k.c_hop; a.c_diag = (R)(5.0 - h->M5); a.mass = (R)k.mass;
     a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c;
     const int K = h->Ls / Prec<R>::VL;
-    const long long nblk = h->V4h * k.nrhs;                                  // (site, rhs) blocks per parity
-    long long threads = nblk * K;
-    if (k.nslots == 2) threads = 2 * ((nblk + a.chunk_blocks - 1) / a.chunk_blocks) * a.chunk_blocks * K;
-    dim3 grid((unsigned)((threads + 127) / 128));
+    a.GS = std::min(HOP_THREADS / 8, HOP_THREADS / K);                                             // sites per CTA
+    a.ngroups = (h->V4h + a.GS - 1) / a.GS;
+    a.chunk_groups = std::max<long long>(1, h->blk_sites / a.GS);             // parity interleave unit = one lattice block
+    long long groups = a.ngroups;
+    if (k.nslots == 2) groups = 2 * ((a.ngroups + a.chunk_groups - 1) / a.chunk_groups) * a.chunk_groups;
     cudaStream_t st = h->stream;
-#define HOPK(LS, DAG, HOP, SELF, G5, AX) hop_kernel<R, LS, DAG, HOP, SELF, G5, AX><<<grid, 128, 0, st>>>(a)
+#define HOPK(LS, DAG, HOP, SELF, G5, AX) hop_kernel<R, LS, DAG, HOP, SELF, G5, AX><<<grid, HOP_THREADS, 0, st>>>(a)
 #define HOPM(LS) \
     switch (k.mode) { \
         case HM_HOP:               if (k.dag) HOPK(LS, true, true, false, false, false); else HOPK(LS, false, true, false, false, false); break; \
@@ -262,14 +271,21 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
         case HM_SELF:              if (k.dag) HOPK(LS, true, false, true, false, false); else HOPK(LS, false, false, true, false, false); break; \
         default: FAIL(h, DWF_EINVAL, "bad hop mode"); \
     }
-    switch (h->Ls) {                     // compile-time Ls for the production sizes, runtime Ls otherwise
-        case 16: HOPM(16); break;
-        case 24: HOPM(24); break;
-        default: HOPM(0); break;
+    // Right-hand sides are processed in chunks (one launch each) so that the working set of a chunk keeps
+    // the L2 reuse of the single-rhs case; CTAs of one chunk run tile-major, rhs-minor.
+    const int RC = h->rhs_chunk;
+    for (int r0 = 0; r0 < k.nrhs; r0 += RC) {
+        a.r0 = r0; a.rn = std::min(RC, k.nrhs - r0);
+        dim3 grid((unsigned)(groups * a.rn));
+        switch (h->Ls) {                 // compile-time Ls for the production sizes, runtime Ls otherwise
+            case 16: HOPM(16); break;
+            case 24: HOPM(24); break;
+            default: HOPM(0); break;
+        }
+        LAUNCH_CHECK(h);
     }
 #undef HOPM
 #undef HOPK
-    LAUNCH_CHECK(h);
     return DWF_OK;
 }
 static int launch_hop(dwf_ctx* h, const HopCall& k) {

@@ -18,6 +18,10 @@
 
 namespace dwf {
 
+#ifndef HOP_THREADS
+#define HOP_THREADS 128       // threads per CTA of the stencil kernel (a CTA covers HOP_THREADS / K sites)
+#endif
+
 template <typename R> struct HopArgs {
     using G = typename Prec<R>::G;
     const G* in_hop[2];    // [p] half field of parity 1-p that feeds output parity p
@@ -29,9 +33,12 @@ template <typename R> struct HopArgs {
     const int* nbr[2];     // [p] neighbour table of parity-p sites: [V4h][8], slot 2mu = +mu, 2mu+1 = -mu
     long long V4h;
     int Ls, nrhs;          // runtime Ls (used when the kernel's LS template parameter is 0)
+    int r0, rn;            // this launch covers right-hand sides r0 .. r0+rn-1
     int parity0;           // output parity of slot 0
-    int nslots;            // 1: one output parity; 2: both, interleaved in chunks of chunk_blocks (site,rhs) blocks
-    long long chunk_blocks;
+    int nslots;            // 1: one output parity; 2: both, interleaved in chunks of chunk_groups site groups
+    int GS;                // sites per CTA (a CTA = one group of G consecutive sites x one rhs x K lane groups)
+    long long ngroups;     // ceil(V4h / G)
+    long long chunk_groups;
     R c_hop, c_diag, mass;
     R ax_a, ax_b, ax_c;
 };
@@ -57,21 +64,28 @@ __device__ __forceinline__ void su3_mul(const R (&u)[18], const CV<V> (&h)[3], C
 
 // One direction of the stencil.  MU = 0..3 (x,y,z,t); SG = -1: projector (1 - gamma_mu), +1: (1 + gamma_mu)
 // (chiral basis R1; the rank-2 forms below are the rows of the 4x4 matrices written out).
+// shared-memory link slot: 16-byte aligned, LINK_SLOT reals (fp32: 18 reals padded to 20; fp64: 18)
+template <typename R> struct LinkSmem;
+template <> struct LinkSmem<float>  { static constexpr int SLOT = 20; static constexpr int SITE = 8 * 20 + 4; };   // 656 B per site
+template <> struct LinkSmem<double> { static constexpr int SLOT = 18; static constexpr int SITE = 8 * 18 + 2; };   // 1168 B per site
+
 template <int MU, int SG, bool FWD, typename R, typename V, typename G>
 __device__ __forceinline__ void hop_dir(CV<V> (&acc)[12], const G* __restrict__ psi, const int cstride,
-                                        const R* __restrict__ link) {
+                                        const R* __restrict__ link /* shared memory */) {
     CV<V> p[12];
 #pragma unroll
     for (int c = 0; c < 12; c++) p[c] = unpack(ldg_nc(psi + c * cstride));
     R u[18];
     if constexpr (sizeof(R) == 4) {
-        const float2* l2 = reinterpret_cast<const float2*>(link);
+        const float4* l4 = reinterpret_cast<const float4*>(link);
 #pragma unroll
-        for (int k = 0; k < 9; k++) { float2 t = __ldg(l2 + k); u[2 * k] = t.x; u[2 * k + 1] = t.y; }
+        for (int k = 0; k < 4; k++) { float4 t = l4[k]; u[4 * k] = t.x; u[4 * k + 1] = t.y; u[4 * k + 2] = t.z; u[4 * k + 3] = t.w; }
+        const float2 t2 = *reinterpret_cast<const float2*>(link + 16);
+        u[16] = t2.x; u[17] = t2.y;
     } else {
         const double2* l2 = reinterpret_cast<const double2*>(link);
 #pragma unroll
-        for (int k = 0; k < 9; k++) { double2 t = __ldg(l2 + k); u[2 * k] = t.x; u[2 * k + 1] = t.y; }
+        for (int k = 0; k < 9; k++) { double2 t = l2[k]; u[2 * k] = t.x; u[2 * k + 1] = t.y; }
     }
     CV<V> h0[3], h1[3], g0[3], g1[3];
 #pragma unroll
@@ -130,17 +144,26 @@ __device__ __forceinline__ void self_term(CV<float2> (&res)[12], const float4* _
     const float4* own_p = blk + k;
     const float4* dn_p = blk + kprev;
     const float4* up_p = blk + knext;
+    // When K divides 32 the K threads of a block sit in one warp: fetch the s-1 / s+1 lanes by shuffle.
+    const bool shfl = (K == 4 || K == 8 || K == 16 || K == 32);
+    const int lane = threadIdx.x & 31;
+    const unsigned mask = __activemask();                    // whole K-groups leave together, sources stay in-group
+    const int src_dn = lane - k + kprev, src_up = lane - k + knext;
 #pragma unroll
     for (int c = 0; c < 12; c++) {
         const CV<float2> own = unpack(ldg_nc(own_p + c * K));
         const bool down = DAG ? (c >= 6) : (c < 6);          // couples to s-1 ?
         CV<float2> t; float2 coef;
         if (down) {
-            const CV<float2> o = unpack(ldg_nc(dn_p + c * K));
-            t.re = make_float2(o.re.y, own.re.x); t.im = make_float2(o.im.y, own.im.x); coef = coef_dn;
+            float oy_re, oy_im;
+            if (shfl) { oy_re = __shfl_sync(mask, own.re.y, src_dn); oy_im = __shfl_sync(mask, own.im.y, src_dn); }
+            else { const CV<float2> o = unpack(ldg_nc(dn_p + c * K)); oy_re = o.re.y; oy_im = o.im.y; }
+            t.re = make_float2(oy_re, own.re.x); t.im = make_float2(oy_im, own.im.x); coef = coef_dn;
         } else {
-            const CV<float2> o = unpack(ldg_nc(up_p + c * K));
-            t.re = make_float2(own.re.y, o.re.x); t.im = make_float2(own.im.y, o.im.x); coef = coef_up;
+            float ox_re, ox_im;
+            if (shfl) { ox_re = __shfl_sync(mask, own.re.x, src_up); ox_im = __shfl_sync(mask, own.im.x, src_up); }
+            else { const CV<float2> o = unpack(ldg_nc(up_p + c * K)); ox_re = o.re.x; ox_im = o.im.x; }
+            t.re = make_float2(own.re.y, ox_re); t.im = make_float2(own.im.y, ox_im); coef = coef_up;
         }
         res[c].re = vfma2(coef, t.re, vfma(c_diag, own.re, res[c].re));
         res[c].im = vfma2(coef, t.im, vfma(c_diag, own.im, res[c].im));
@@ -168,50 +191,82 @@ __device__ __forceinline__ void self_term(CV<double> (&res)[12], const double2* 
 
 // Gamma5 = gamma5 R5 (eq. 6, R6): lane group k of a block goes to group K-1-k (fp32: the two lanes
 // of the group also swap).
+//
+// Work decomposition: a CTA of 256 threads handles G = 256/K consecutive sites (one tile of the native
+// site order) for ONE right-hand side; thread = (site in tile, lane group k).  The 8 links of each of
+// the G sites are fetched once per CTA into shared memory and read back as 128-bit broadcasts.
 template <typename R, int LS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY>
-__global__ void __launch_bounds__(128, 4)
+__global__ void __launch_bounds__(HOP_THREADS, 512 / HOP_THREADS)
 hop_kernel(const HopArgs<R> a) {
     using V = typename Prec<R>::V;
     using G = typename Prec<R>::G;
     constexpr int VL = Prec<R>::VL;
+    constexpr int SLOT = LinkSmem<R>::SLOT, SITE = LinkSmem<R>::SITE;
     const int K = (LS > 0) ? LS / VL : a.Ls / VL;            // lane groups per component of a (site, rhs) block
-    // ---- which (output parity slot, site, rhs, lane group) is this thread? ------------------------------
-    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    long long blk = gid / K;                                  // (site, rhs) block index, maybe across both slots
-    const int k = (int)(gid - blk * K);
+    __shared__ __align__(16) R s_link[HOP ? (HOP_THREADS / 8) * SITE : 4];
+
+    // ---- which (output parity slot, site group, rhs) is this CTA? -------------------------------------
+    long long gg = (long long)blockIdx.x / a.rn;              // site group, maybe across both slots
+    const int r = a.r0 + (int)(blockIdx.x - gg * a.rn);
     int pi = 0;
-    if (a.nslots == 2) {                                      // chunks of chunk_blocks alternate between the parities
-        const long long q = blk / (2 * a.chunk_blocks);
-        const long long rem = blk - q * 2 * a.chunk_blocks;
-        pi = rem >= a.chunk_blocks;
-        blk = q * a.chunk_blocks + (rem - pi * a.chunk_blocks);
+    if (a.nslots == 2) {                                      // chunks of chunk_groups alternate between the parities
+        const long long q = gg / (2 * a.chunk_groups);
+        const long long rem = gg - q * 2 * a.chunk_groups;
+        pi = rem >= a.chunk_groups;
+        gg = q * a.chunk_groups + (rem - pi * a.chunk_groups);
     }
-    const long long site = blk / a.nrhs;
-    if (site >= a.V4h) return;
-    const int r = (int)(blk - site * a.nrhs);
-    const int BS = 12 * K;                                    // groups per block
+    if (gg >= a.ngroups) return;                              // uniform over the CTA
+    const int p = (a.parity0 + pi) & 1;
+    const long long site0 = gg * a.GS;
+
+    if constexpr (HOP) {                                      // cooperative link fetch: thread t -> (site t/8, direction t%8)
+        const int ls = threadIdx.x >> 3, d = threadIdx.x & 7;
+        const long long st = site0 + ls;
+        if (ls < a.GS && st < a.V4h) {
+            const R* src;
+            if ((d & 1) == 0) src = a.gauge[p] + (size_t)st * 72 + (d >> 1) * 18;
+            else { const int n = __ldg(a.nbr[pi] + st * 8 + d); src = a.gauge[p ^ 1] + (size_t)n * 72 + (d >> 1) * 18; }
+            R* dst = s_link + ls * SITE + d * SLOT;
+            if constexpr (sizeof(R) == 4) {
+                const float2* s2 = reinterpret_cast<const float2*>(src);
+                float2* d2 = reinterpret_cast<float2*>(dst);
+#pragma unroll
+                for (int j = 0; j < 9; j++) d2[j] = __ldg(s2 + j);
+            } else {
+                const double2* s2 = reinterpret_cast<const double2*>(src);
+                double2* d2 = reinterpret_cast<double2*>(dst);
+#pragma unroll
+                for (int j = 0; j < 9; j++) d2[j] = __ldg(s2 + j);
+            }
+        }
+        __syncthreads();
+    }
+    const int ls = threadIdx.x / K;                           // site within the tile
+    const int k = threadIdx.x - ls * K;
+    const long long site = site0 + ls;
+    if (ls >= a.GS || site >= a.V4h) return;
+    const int BS = 12 * K;                                    // groups per (site, rhs) block
+    const long long blk = site * a.nrhs + r;
 
     CV<V> acc[12];
 #pragma unroll
     for (int c = 0; c < 12; c++) { acc[c].re = vzero(V()); acc[c].im = vzero(V()); }
 
     if constexpr (HOP) {
-        const int p = (a.parity0 + pi) & 1;
         const int4* nb4 = reinterpret_cast<const int4*>(a.nbr[pi] + site * 8);
         const int4 n0 = __ldg(nb4), n1 = __ldg(nb4 + 1);
         const G* in = a.in_hop[pi] + (size_t)r * BS + k;
         const size_t sstride = (size_t)a.nrhs * BS;           // groups per site
-        const R* u_own = a.gauge[p] + (size_t)site * 72;
-        const R* u_nbr = a.gauge[p ^ 1];
+        const R* u = s_link + ls * SITE;
         constexpr int SF = DAG ? +1 : -1;                     // projector sign on the forward hop
-        hop_dir<0, SF, true >(acc, in + (size_t)n0.x * sstride, K, u_own + 0);
-        hop_dir<0, -SF, false>(acc, in + (size_t)n0.y * sstride, K, u_nbr + (size_t)n0.y * 72 + 0);
-        hop_dir<1, SF, true >(acc, in + (size_t)n0.z * sstride, K, u_own + 18);
-        hop_dir<1, -SF, false>(acc, in + (size_t)n0.w * sstride, K, u_nbr + (size_t)n0.w * 72 + 18);
-        hop_dir<2, SF, true >(acc, in + (size_t)n1.x * sstride, K, u_own + 36);
-        hop_dir<2, -SF, false>(acc, in + (size_t)n1.y * sstride, K, u_nbr + (size_t)n1.y * 72 + 36);
-        hop_dir<3, SF, true >(acc, in + (size_t)n1.z * sstride, K, u_own + 54);
-        hop_dir<3, -SF, false>(acc, in + (size_t)n1.w * sstride, K, u_nbr + (size_t)n1.w * 72 + 54);
+        hop_dir<0, SF, true >(acc, in + (size_t)n0.x * sstride, K, u + 0 * SLOT);
+        hop_dir<0, -SF, false>(acc, in + (size_t)n0.y * sstride, K, u + 1 * SLOT);
+        hop_dir<1, SF, true >(acc, in + (size_t)n0.z * sstride, K, u + 2 * SLOT);
+        hop_dir<1, -SF, false>(acc, in + (size_t)n0.w * sstride, K, u + 3 * SLOT);
+        hop_dir<2, SF, true >(acc, in + (size_t)n1.x * sstride, K, u + 4 * SLOT);
+        hop_dir<2, -SF, false>(acc, in + (size_t)n1.y * sstride, K, u + 5 * SLOT);
+        hop_dir<3, SF, true >(acc, in + (size_t)n1.z * sstride, K, u + 6 * SLOT);
+        hop_dir<3, -SF, false>(acc, in + (size_t)n1.w * sstride, K, u + 7 * SLOT);
 #pragma unroll
         for (int c = 0; c < 12; c++) { acc[c].re = vmul(a.c_hop, acc[c].re); acc[c].im = vmul(a.c_hop, acc[c].im); }
     }
