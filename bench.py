@@ -158,10 +158,12 @@ def run_only(args, dev):
     import dwf_inputs as gen
     from paper_2103_05034_b200 import DWF_DDW, DWF_DHOP, DWF_F32, DWF_F64, DWF_HDW, DWF_SCHUR_EO, Dwf
     f32 = args.prec == "f32"
+    name = args.only
+    if name.endswith("_48"):
+        return run_only_config4(args, dev)
     d = Dwf(L, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)
     d.set_gauge(torch.from_numpy(gen.gauge_random(L, 1002)).to(d.cdtype).to(dev))
     g = torch.Generator(device=dev); g.manual_seed(2002)
-    name = args.only
     nrhs = int(name.split("nrhs")[1]) if "nrhs" in name else (CHEB_NVEC if name == "chebyshev" else 1)
     d.set_workspace(nrhs)
     half = name.startswith("schur") or name == "cg"
@@ -191,6 +193,42 @@ def run_only(args, dev):
         by = apply_bytes(nrhs, 4 if f32 else 8)
         out.update({"GB/s": round(by / ms / 1e6, 1), "GFlop/s": round(FLOP_PER_SITE * V5 * nrhs / ms / 1e6, 1),
                     "frac_of_hbm_peak": round(by / ms / 1e6 / peaks()[0], 4)})
+    print(json.dumps(out), flush=True)
+
+
+def run_only_config4(args, dev):
+    """BASELINE.json configs[4]: 48^3 x 96 x Ls=24 fp32, m = 0.00078: one D_DW apply / 100 rb-CG iterations."""
+    import torch
+
+    import dwf_inputs as gen
+    from paper_2103_05034_b200 import DWF_DDW, DWF_F32, Dwf
+    L4, LS4, MASS4 = (48, 48, 48, 96), 24, 0.00078
+    v5 = L4[0] * L4[1] * L4[2] * L4[3] * LS4
+    d = Dwf(L4, LS4, M5, MASS4, DWF_F32, device=dev)
+    d.set_gauge(gen.gauge_random_torch(L4, 1004, dev, torch.complex64))
+    g = torch.Generator(device=dev); g.manual_seed(2004)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if args.only == "ddw_48":
+        x, y = d.field(1).normal_(generator=g), d.field(1)
+        for _ in range(max(args.warmup, 3)):
+            d.apply(DWF_DDW, x, y, 1)
+        a.record()
+        for _ in range(args.steps):
+            d.apply(DWF_DDW, x, y, 1)
+        b.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / args.steps
+        by = v5 * (48.0 * 4 + 72.0 * 4 / LS4)
+        out = {"only": "ddw_48", "ms": round(ms, 3), "GB/s": round(by / ms / 1e6, 1), "GFlop/s": round(FLOP_PER_SITE * v5 / ms / 1e6, 1),
+               "frac_of_hbm_peak": round(by / ms / 1e6 / peaks()[0], 4)}
+    else:
+        d.set_workspace(1)
+        bb, xx = d.field(1, half=True).normal_(generator=g), d.field(1, half=True, zero=True)
+        d.cg_schur(bb, xx, 3)
+        xx.zero_(); torch.cuda.synchronize()
+        a.record(); hist = d.cg_schur(bb, xx, 100); b.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(b)
+        out = {"only": "cg_48", "iters": 100, "ms": round(ms, 2), "iterations/s": round(101 / ms * 1e3, 2),
+               "resid2_first_last": [hist[0], hist[-1]]}
     print(json.dumps(out), flush=True)
 
 

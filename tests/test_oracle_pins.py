@@ -232,3 +232,42 @@ def test_blas1(oracle, fields):
     want = np.array([np.vdot(x[r], y[r]) for r in range(2)])
     assert np.max(np.abs(oracle.inner(x, y) - want) / np.abs(want)) < 1e-13
     assert np.max(np.abs(oracle.norm2(x) - np.array([np.sum(np.abs(x[r]) ** 2) for r in range(2)]))) < 1e-8
+
+
+# ---------------------------------------------------------------- site-list mode (used at configs[4])
+def _gather(L, U, psi, sites):
+    """Neighbourhoods in the layout oracle.ddw_sites expects (harness code: indexing only)."""
+    n, Ls = len(sites), psi.shape[1]
+    nbr = np.zeros((n, 9, Ls, 4, 3), dtype=complex); links = np.zeros((n, 8, 3, 3), dtype=complex)
+    for i, c in enumerate(sites):
+        x, y, z, t = c
+        nbr[i, 0] = psi[0, :, t, z, y, x]
+        for mu in range(4):
+            for j, d in enumerate((+1, -1)):
+                m = list(c); m[mu] = (m[mu] + d) % L[mu]
+                nbr[i, 1 + 2 * mu + j] = psi[0, :, m[3], m[2], m[1], m[0]]
+                src = c if d > 0 else m
+                links[i, 2 * mu + j] = U[mu, src[3], src[2], src[1], src[0]]
+    return nbr, links
+
+
+def test_site_list_mode(oracle):
+    """ddw_sites against (i) the hand-derived golden example and (ii) the pinned full-volume D_DW at every site."""
+    L, Ls = (4, 4, 4, 4), 8
+    sites = [(x, y, z, t) for t in range(4) for z in range(4) for y in range(4) for x in range(4)]
+    U = gen.gauge_unit(L)
+    src = gen.point_source(L, Ls, (0, 0, 0, 0), 0, 0, 0)
+    nbr, links = _gather(L, U, src, sites)
+    got = oracle.ddw_sites(L, Ls, M5, MASS, np.array(sites, dtype=np.int32), nbr, links)
+    expect = np.zeros_like(got)
+    for s_, s, (x, y, z, t), spin, val in _read_golden():
+        if s_ == "A":
+            expect[sites.index((x, y, z, t)), s, spin, 0] = val
+    assert np.max(np.abs(got - expect)) < 1e-15
+    U = gen.gauge_random(L, 1000)
+    psi = gen.spinor_gaussian(L, Ls, 1, 2000)
+    nbr, links = _gather(L, U, psi, sites)
+    got = oracle.ddw_sites(L, Ls, M5, MASS, np.array(sites, dtype=np.int32), nbr, links)
+    full = oracle.ddw(U, psi, M5, MASS)[0]
+    want = np.stack([full[:, t, z, y, x] for (x, y, z, t) in sites])
+    assert rel(got, want) < 1e-15
