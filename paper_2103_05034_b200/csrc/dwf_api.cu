@@ -14,6 +14,7 @@
 #include "../../include/dwf.h"
 #include "dwf_aux.cuh"
 #include "dwf_hop.cuh"
+#include "dwf_tile.cuh"
 
 using namespace dwf;
 
@@ -23,6 +24,7 @@ struct dwf_ctx {
     long long V4, V4h;
     cudaStream_t stream;
     void* gauge;          // native links [2][V4h][4][18] reals
+    void* glinks;         // gathered, (-1/2)-scaled links for the tiled stencil (tile_sites != 0)
     int* nbr;             // [2][V4h][8]
     int* lex;             // [2][V4h]
     bool have_gauge;
@@ -32,6 +34,8 @@ struct dwf_ctx {
     double* scal_host;    // pinned mirror
     int sm_count;
     long long blk_sites;  // sites per parity in one lattice block of the native site order
+    int tile_sites;       // sites per parity in one tile of the native site order (0: lattice is not made of whole tiles)
+    int sg_shift;         // block order [site group][rhs][site in group]: log2(group size)
     int rhs_chunk;        // right-hand sides per stencil launch
     long long launches;
     char err[256];
@@ -56,6 +60,7 @@ static inline long long half_groups(const dwf_ctx* h, int nrhs) {
     return h->V4h * 12 * ((long long)nrhs * h->Ls / vl(h));
 }
 static inline int block_groups(const dwf_ctx* h) { return 12 * h->Ls / vl(h); }   // groups per (site, rhs) block
+static inline int run_groups(const dwf_ctx* h) { return block_groups(h) << h->sg_shift; }   // groups per contiguous run of one rhs
 
 // ------------------------------------------------------------------------------------------------
 // Index tables.  Native site order within a parity: 4D blocks of BLK^4 sites in lexicographic block
@@ -65,7 +70,9 @@ static inline int block_groups(const dwf_ctx* h) { return 12 * h->Ls / vl(h); } 
 static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nbr) {
     const int* L = h->L;
     int B[4] = {4, 4, 4, 4};      // outer block: unit of the parity interleave, L2 locality
-    int T[4] = {4, 4, 2, 2};      // inner tile : 32 sites per parity = what one CTA works on (L1 locality)
+    int T[4] = {4, 4, 2, 2};      // inner tile : 32 sites per parity = what one CTA of the tiled stencil works on
+    // the tile interior of one rhs must fit shared memory twice per SM: 16-site tiles for wide blocks
+    if ((size_t)h->Ls * 96 * real_bytes(h) / 4 > 1536) T[1] = 2;
     auto parse = [](const char* name, int* v) {
         if (const char* env = getenv(name)) { int b[4]; if (sscanf(env, "%d,%d,%d,%d", &b[0], &b[1], &b[2], &b[3]) == 4) for (int i = 0; i < 4; i++) v[i] = b[i]; }
     };
@@ -76,6 +83,12 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     if ((T[0] * T[1] * T[2] * T[3]) % 2 != 0) for (int i = 0; i < 4; i++) T[i] = B[i];
     const long long V4 = h->V4, V4h = h->V4h;
     h->blk_sites = (long long)B[0] * B[1] * B[2] * B[3] / 2;
+    const int tsites = T[0] * T[1] * T[2] * T[3] / 2;
+    bool whole = true;
+    for (int i = 0; i < 4; i++) whole = whole && (L[i] % T[i] == 0);
+    h->tile_sites = (whole && (tsites == 16 || tsites == 32)) ? tsites : 0;
+    h->sg_shift = h->tile_sites == 32 ? 5 : h->tile_sites == 16 ? 4 : 0;
+    if (getenv("DWF_NO_TILE")) h->tile_sites = 0;             // keeps the block order, uses the generic kernel
     lex.assign(2 * V4h, 0);
     std::vector<int> idx_of(V4);                                                // lex site -> index within its parity
     long long cnt[2] = {0, 0};
@@ -132,7 +145,9 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
     h->rhs_chunk = 4;
     if (const char* env = getenv("DWF_RHS_CHUNK")) h->rhs_chunk = std::max(1, atoi(env));
     const size_t gbytes = (size_t)2 * h->V4h * 72 * real_bytes(h);
+    const size_t glbytes = (size_t)2 * h->V4h * (144 * real_bytes(h) + 16);
     bool ok = cudaMalloc(&h->gauge, gbytes) == cudaSuccess
+           && (h->tile_sites == 0 || (cudaMalloc(&h->glinks, glbytes) == cudaSuccess && cudaMemset(h->glinks, 0, glbytes) == cudaSuccess))
            && cudaMalloc((void**)&h->nbr, nbr.size() * sizeof(int)) == cudaSuccess
            && cudaMalloc((void**)&h->lex, lex.size() * sizeof(int)) == cudaSuccess
            && cudaMalloc((void**)&h->partial, (size_t)MAX_RED_BLOCKS * MAX_NRHS * 2 * sizeof(double)) == cudaSuccess
@@ -147,7 +162,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
 
 extern "C" int dwf_destroy(dwf_handle h) {
     if (!h) return DWF_EINVAL;
-    cudaFree(h->gauge); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal);
+    cudaFree(h->gauge); cudaFree(h->glinks); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal);
     if (h->scal_host) cudaFreeHost(h->scal_host);
     delete h;
     return DWF_OK;
@@ -192,6 +207,13 @@ extern "C" int dwf_set_gauge(dwf_handle h, const void* U) {
     if (h->prec == DWF_F32) reorder_gauge_kernel<float><<<blocks, 256, 0, h->stream>>>((const float*)U, (float*)h->gauge, h->lex, h->V4h, h->V4, spatial, h->L[3]);
     else                    reorder_gauge_kernel<double><<<blocks, 256, 0, h->stream>>>((const double*)U, (double*)h->gauge, h->lex, h->V4h, h->V4, spatial, h->L[3]);
     LAUNCH_CHECK(h);
+    if (h->glinks) {
+        const long long m = 2 * h->V4h * 144;
+        const unsigned gb = (unsigned)((m + 255) / 256);
+        if (h->prec == DWF_F32) gather_links_kernel<float><<<gb, 256, 0, h->stream>>>((const float*)h->gauge, (float*)h->glinks, h->nbr, h->V4h, TileLinks<float>::SITE);
+        else                    gather_links_kernel<double><<<gb, 256, 0, h->stream>>>((const double*)h->gauge, (double*)h->glinks, h->nbr, h->V4h, TileLinks<double>::SITE);
+        LAUNCH_CHECK(h);
+    }
     h->have_gauge = true;
     return DWF_OK;
 }
@@ -204,7 +226,7 @@ static int reorder_spinor(dwf_ctx* h, const void* canon_in, void* canon_out, voi
     if (parity < 0) { n0 = (G*)native; n1 = (G*)native + per_parity; l0 = h->lex; l1 = h->lex + h->V4h; ny = 2; }
     else            { n0 = n1 = (G*)native; l0 = l1 = h->lex + (size_t)parity * h->V4h; ny = 1; }
     dim3 grid((unsigned)((per_parity + 255) / 256), ny);
-    reorder_spinor_kernel<R, IMPORT><<<grid, 256, 0, h->stream>>>((const R*)canon_in, (R*)canon_out, n0, n1, l0, l1, h->V4h, h->V4, h->Ls, nrhs);
+    reorder_spinor_kernel<R, IMPORT><<<grid, 256, 0, h->stream>>>((const R*)canon_in, (R*)canon_out, n0, n1, l0, l1, h->V4h, h->V4, h->Ls, nrhs, h->sg_shift);
     LAUNCH_CHECK(h);
     return DWF_OK;
 }
@@ -255,13 +277,28 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.c_hop = (R)k.c_hop; a.c_diag = (R)(5.0 - h->M5); a.mass = (R)k.mass;
     a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c;
     const int K = h->Ls / Prec<R>::VL;
-    a.GS = std::min(HOP_THREADS / 8, HOP_THREADS / K);                                             // sites per CTA
+    // tiled persistent stencil (dwf_tile.cuh): lattice made of whole tiles, compile-time Ls, a hop to do
+    const bool ls_ct = (h->Ls == 16 || h->Ls == 24);
+    const int TS = (ls_ct && k.mode != HM_SELF && h->glinks) ? h->tile_sites : 0;
+    a.sg_shift = h->sg_shift;
+    a.GS = TS ? TS : std::min(HOP_THREADS / 8, HOP_THREADS / K);                                   // sites per CTA
     a.ngroups = (h->V4h + a.GS - 1) / a.GS;
     a.chunk_groups = std::max<long long>(1, h->blk_sites / a.GS);             // parity interleave unit = one lattice block
     long long groups = a.ngroups;
     if (k.nslots == 2) groups = 2 * ((a.ngroups + a.chunk_groups - 1) / a.chunk_groups) * a.chunk_groups;
     cudaStream_t st = h->stream;
+    const size_t lsite = 144 * sizeof(R) + 16;
+    a.glinks[0] = (const R*)h->glinks;
+    a.glinks[1] = (const R*)((const char*)h->glinks + (size_t)h->V4h * lsite);
+    a.sigma = (R)(-2.0 * k.c_hop);                                             // links carry the factor -1/2
 #define HOPK(LS, DAG, HOP, SELF, G5, AX) hop_kernel<R, LS, DAG, HOP, SELF, G5, AX><<<grid, HOP_THREADS, 0, st>>>(a)
+#define TILEK(LS, TSV, DAG, SELF, G5, AX) do { \
+        using TG = TileGeom<R, LS, TSV>; \
+        auto kern = hop_tile_kernel<R, LS, TSV, DAG, true, SELF, G5, AX>; \
+        cudaError_t e_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TG::SMEM_BYTES); \
+        if (e_ != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e_)); \
+        const long long ctas = std::min<long long>(a.nitems, (long long)h->sm_count * TG::MIN_CTAS); \
+        kern<<<(unsigned)ctas, TG::THREADS, TG::SMEM_BYTES, st>>>(a); } while (0)
 #define HOPM(LS) \
     switch (k.mode) { \
         case HM_HOP:               if (k.dag) HOPK(LS, true, true, false, false, false); else HOPK(LS, false, true, false, false, false); break; \
@@ -271,19 +308,29 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
         case HM_SELF:              if (k.dag) HOPK(LS, true, false, true, false, false); else HOPK(LS, false, false, true, false, false); break; \
         default: FAIL(h, DWF_EINVAL, "bad hop mode"); \
     }
+#define TILEM(LS, TSV) \
+    switch (k.mode) { \
+        case HM_HOP:               if (k.dag) TILEK(LS, TSV, true, false, false, false); else TILEK(LS, TSV, false, false, false, false); break; \
+        case HM_HOP_SELF:          if (k.dag) TILEK(LS, TSV, true, true, false, false);  else TILEK(LS, TSV, false, true, false, false); break; \
+        case HM_HOP_SELF_G5:       TILEK(LS, TSV, false, true, true, false); break; \
+        case HM_HOP_SELF_G5_AXPBY: TILEK(LS, TSV, false, true, true, true); break; \
+        default: FAIL(h, DWF_EINVAL, "bad hop mode"); \
+    }
     // Right-hand sides are processed in chunks (one launch each) so that the working set of a chunk keeps
     // the L2 reuse of the single-rhs case; CTAs of one chunk run tile-major, rhs-minor.
     const int RC = h->rhs_chunk;
     for (int r0 = 0; r0 < k.nrhs; r0 += RC) {
         a.r0 = r0; a.rn = std::min(RC, k.nrhs - r0);
+        a.nitems = groups * a.rn;
         dim3 grid((unsigned)(groups * a.rn));
-        switch (h->Ls) {                 // compile-time Ls for the production sizes, runtime Ls otherwise
-            case 16: HOPM(16); break;
-            case 24: HOPM(24); break;
-            default: HOPM(0); break;
-        }
+        // compile-time Ls for the production sizes (tiled when the lattice allows), runtime Ls otherwise
+        if (h->Ls == 16)      { if (TS == 32) { TILEM(16, 32) } else if (TS == 16) { TILEM(16, 16) } else { HOPM(16) } }
+        else if (h->Ls == 24) { if (TS == 16) { TILEM(24, 16) } else { HOPM(24) } }
+        else { HOPM(0) }
         LAUNCH_CHECK(h);
     }
+#undef TILEM
+#undef TILEK
 #undef HOPM
 #undef HOPK
     return DWF_OK;
@@ -299,7 +346,7 @@ static int launch_mooinv_t(dwf_ctx* h, const void* in, void* out, int nrhs, doub
     const double v0scale = kappa / (1.0 + mass * std::pow(kappa, (double)h->Ls));
     const long long threads = h->V4h * 12 * nrhs;
     const unsigned blocks = (unsigned)((threads + 127) / 128);
-#define MOOK(LS) mooinv_kernel<R, LS, DAG><<<blocks, 128, 0, h->stream>>>((const G*)in, (G*)out, h->V4h, nrhs, (R)kappa, (R)mass, (R)v0scale)
+#define MOOK(LS) mooinv_kernel<R, LS, DAG><<<blocks, 128, 0, h->stream>>>((const G*)in, (G*)out, h->V4h, nrhs, h->sg_shift, (R)kappa, (R)mass, (R)v0scale)
     switch (h->Ls) {
         case 4: MOOK(4); break;   case 8: MOOK(8); break;   case 12: MOOK(12); break;
         case 16: MOOK(16); break; case 24: MOOK(24); break; case 32: MOOK(32); break;
@@ -429,7 +476,7 @@ static unsigned blas_blocks(const dwf_ctx* h, long long ngroups, long long perio
 
 static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp) {
     const long long ng = half_groups(h, nrhs) * (half ? 1 : 2);
-    const int BS = block_groups(h);
+    const int BS = run_groups(h);
     const unsigned blocks = blas_blocks(h, ng, (long long)BS * nrhs);
     if (h->prec == DWF_F32) {
         if (norm) inner_kernel<float, true><<<blocks, 256, 0, h->stream>>>((const float4*)x, nullptr, ng, BS, nrhs, h->partial);
@@ -452,7 +499,7 @@ extern "C" int dwf_axpy(dwf_handle h, const double* a_host, const void* x, void*
     RhsCoef a;
     for (int r = 0; r < nrhs; r++) { a.re[r] = a_host[2 * r]; a.im[r] = a_host[2 * r + 1]; }
     const long long ng = half_groups(h, nrhs) * (half ? 1 : 2);
-    const int BS = block_groups(h);
+    const int BS = run_groups(h);
     const unsigned blocks = blas_blocks(h, ng, (long long)BS * nrhs);
     if (h->prec == DWF_F32) axpy_kernel<float><<<blocks, 256, 0, h->stream>>>((const float4*)x, (float4*)y, ng, BS, nrhs, a);
     else                    axpy_kernel<double><<<blocks, 256, 0, h->stream>>>((const double2*)x, (double2*)y, ng, BS, nrhs, a);

@@ -7,14 +7,14 @@ namespace dwf {
 
 // ------------------------------------------------------------------------------------------------
 // a1. canonical <-> native reorder.  canonical spinor: complex<R> [nrhs][Ls][V4 lex][12];
-// native: group index (((site*nrhs + r)*12 + c)*K + k), K = Ls/VL, group k holds lanes s = k*VL .. k*VL+VL-1.
+// native: group index ((blk_index(site, r)*12 + c)*K + k), K = Ls/VL, group k holds lanes s = k*VL .. k*VL+VL-1.
 // One thread per native group; blockIdx.y = parity slot.
 // ------------------------------------------------------------------------------------------------
 template <typename R, bool IMPORT>
 __global__ void reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restrict__ canon_out,
                                       typename Prec<R>::G* native0, typename Prec<R>::G* native1,
                                       const int* __restrict__ lex0, const int* __restrict__ lex1,
-                                      long long V4h, long long V4, int Ls, int nrhs) {
+                                      long long V4h, long long V4, int Ls, int nrhs, int sg_shift) {
     using G = typename Prec<R>::G;
     constexpr int VL = Prec<R>::VL;
     const int K = Ls / VL;
@@ -29,7 +29,7 @@ __global__ void reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restr
     const int* lex = blockIdx.y ? lex1 : lex0;
     const long long lx = lex[site];
     const int r = lg / K, k = lg % K, s = k * VL;
-    const size_t nidx = (((size_t)site * nrhs + r) * 12 + c) * K + k;
+    const size_t nidx = ((size_t)blk_index(site, r, nrhs, sg_shift) * 12 + c) * K + k;
     const size_t c0 = ((((size_t)r * Ls + s) * V4 + lx) * 12 + c) * 2;
     const size_t sstride = (size_t)V4 * 12 * 2;          // to the next s
     if constexpr (IMPORT) {
@@ -60,6 +60,26 @@ __global__ void reorder_gauge_kernel(const R* __restrict__ canon, R* __restrict_
     native[gid * 2 + 1] = sign * canon[ci + 1];
 }
 
+// Gathered links for the tiled stencil (dwf_tile.cuh): per site [mu][U_mu(x) 18 | U_mu(x-mu) 18] + padding,
+// pre-scaled by -1/2 (exact), so that a tile's links are one contiguous run and need no index lookup.
+template <typename R>
+__global__ void gather_links_kernel(const R* __restrict__ gauge /*[2][V4h][4][18]*/, R* __restrict__ glinks /*[2][V4h][site_reals]*/,
+                                    const int* __restrict__ nbr /*[2][V4h][8]*/, long long V4h, int site_reals) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= 2 * V4h * 4 * 36) return;
+    const int j = (int)(gid % 36);
+    const int mu = (int)((gid / 36) % 4);
+    const long long ps = gid / 144;                         // p*V4h + site
+    R v;
+    if (j < 18) v = gauge[(ps * 4 + mu) * 18 + j];
+    else {
+        const long long p = ps / V4h;
+        const long long q = (1 - p) * V4h + nbr[ps * 8 + 2 * mu + 1];
+        v = gauge[(q * 4 + mu) * 18 + (j - 18)];
+    }
+    glinks[ps * site_reals + mu * 36 + j] = R(-0.5) * v;
+}
+
 // ------------------------------------------------------------------------------------------------
 // a5. Exact inverse of the 4D-site-diagonal block M_oo = M_ee.  Per site, per
 // complex component, per rhs the Ls x Ls system is cyclic bidiagonal:
@@ -72,7 +92,7 @@ __global__ void reorder_gauge_kernel(const R* __restrict__ canon, R* __restrict_
 // ------------------------------------------------------------------------------------------------
 template <typename R, int LS, bool DAG>
 __global__ void __launch_bounds__(128)
-mooinv_kernel(const typename Prec<R>::G* in, typename Prec<R>::G* out, long long V4h, int nrhs,
+mooinv_kernel(const typename Prec<R>::G* in, typename Prec<R>::G* out, long long V4h, int nrhs, int sg_shift,
               R kappa, R mass, R v0scale /* kappa / (1 + m kappa^Ls) */) {
     using G = typename Prec<R>::G;
     constexpr int VL = Prec<R>::VL;
@@ -82,7 +102,7 @@ mooinv_kernel(const typename Prec<R>::G* in, typename Prec<R>::G* out, long long
     const int r = (int)(gid % nrhs);
     const int c = (int)((gid / nrhs) % 12);
     const long long site = gid / (12 * nrhs);
-    const size_t base = (((size_t)site * nrhs + r) * 12 + c) * NG;
+    const size_t base = ((size_t)blk_index(site, r, nrhs, sg_shift) * 12 + c) * NG;
     const bool down = DAG ? (c >= 6) : (c < 6);
     R bre[LS], bim[LS];
 #pragma unroll
@@ -114,8 +134,8 @@ mooinv_kernel(const typename Prec<R>::G* in, typename Prec<R>::G* out, long long
 }
 
 // ------------------------------------------------------------------------------------------------
-// a7. BLAS-1.  Fields are flat arrays of groups; group e belongs to rhs (e / BS) % nrhs, BS = 12*Ls/VL
-// groups per (site, rhs) block.  Launch geometry guarantees (gridDim.x * blockDim.x) % (BS*nrhs) == 0,
+// a7. BLAS-1.  Fields are flat arrays of groups; group e belongs to rhs (e / BS) % nrhs, BS = groups per
+// run of one rhs (12*Ls/VL groups per (site, rhs) block x sites per site group).  Launch geometry guarantees (gridDim.x * blockDim.x) % (BS*nrhs) == 0,
 // so a thread keeps one rhs for its whole grid-stride loop.  Reductions: fp64 per-thread accumulation, fixed-
 // order in-block combine per rhs, per-block partials, fixed-order final pass => deterministic.
 // ------------------------------------------------------------------------------------------------

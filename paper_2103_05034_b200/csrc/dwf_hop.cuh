@@ -37,6 +37,11 @@ template <typename R> struct HopArgs {
     int parity0;           // output parity of slot 0
     int nslots;            // 1: one output parity; 2: both, interleaved in chunks of chunk_groups site groups
     int GS;                // sites per CTA (a CTA = one group of G consecutive sites x one rhs x K lane groups)
+    int sg_shift;          // log2 of the site-group size of the block order; 0 = [site][rhs]
+    // tiled kernel only (dwf_tile.cuh):
+    const R* glinks[2];    // [p] gathered links of parity-p sites: [site][mu][fwd 18 | bwd 18] x (-1/2), 16 B pad per site
+    R sigma;               // res = sigma * hop' + self  with hop' built from the (-1/2)-scaled links
+    long long nitems;      // work items (tile, rhs, parity slot) of this launch
     long long ngroups;     // ceil(V4h / G)
     long long chunk_groups;
     R c_hop, c_diag, mass;
@@ -69,24 +74,9 @@ template <typename R> struct LinkSmem;
 template <> struct LinkSmem<float>  { static constexpr int SLOT = 20; static constexpr int SITE = 8 * 20 + 4; };   // 656 B per site
 template <> struct LinkSmem<double> { static constexpr int SLOT = 18; static constexpr int SITE = 8 * 18 + 2; };   // 1168 B per site
 
-template <int MU, int SG, bool FWD, typename R, typename V, typename G>
-__device__ __forceinline__ void hop_dir(CV<V> (&acc)[12], const G* __restrict__ psi, const int cstride,
-                                        const R* __restrict__ link /* shared memory */) {
-    CV<V> p[12];
-#pragma unroll
-    for (int c = 0; c < 12; c++) p[c] = unpack(ldg_nc(psi + c * cstride));
-    R u[18];
-    if constexpr (sizeof(R) == 4) {
-        const float4* l4 = reinterpret_cast<const float4*>(link);
-#pragma unroll
-        for (int k = 0; k < 4; k++) { float4 t = l4[k]; u[4 * k] = t.x; u[4 * k + 1] = t.y; u[4 * k + 2] = t.z; u[4 * k + 3] = t.w; }
-        const float2 t2 = *reinterpret_cast<const float2*>(link + 16);
-        u[16] = t2.x; u[17] = t2.y;
-    } else {
-        const double2* l2 = reinterpret_cast<const double2*>(link);
-#pragma unroll
-        for (int k = 0; k < 9; k++) { double2 t = l2[k]; u[2 * k] = t.x; u[2 * k + 1] = t.y; }
-    }
+// core of one direction: project p (12 components) to a half spinor, multiply by the link u, reconstruct, accumulate
+template <int MU, int SG, bool FWD, typename R, typename V>
+__device__ __forceinline__ void hop_dir_core(CV<V> (&acc)[12], const CV<V> (&p)[12], const R (&u)[18]) {
     CV<V> h0[3], h1[3], g0[3], g1[3];
 #pragma unroll
     for (int col = 0; col < 3; col++) {
@@ -125,6 +115,27 @@ __device__ __forceinline__ void hop_dir(CV<V> (&acc)[12], const G* __restrict__ 
             else                  { acc[6 + col] = cadd(acc[6 + col], g0[col]); acc[9 + col] = cadd(acc[9 + col], g1[col]); }
         }
     }
+}
+
+template <int MU, int SG, bool FWD, typename R, typename V, typename G>
+__device__ __forceinline__ void hop_dir(CV<V> (&acc)[12], const G* __restrict__ psi, const int cstride,
+                                        const R* __restrict__ link /* shared memory */) {
+    CV<V> p[12];
+#pragma unroll
+    for (int c = 0; c < 12; c++) p[c] = unpack(ldg_nc(psi + c * cstride));
+    R u[18];
+    if constexpr (sizeof(R) == 4) {
+        const float4* l4 = reinterpret_cast<const float4*>(link);
+#pragma unroll
+        for (int k = 0; k < 4; k++) { float4 t = l4[k]; u[4 * k] = t.x; u[4 * k + 1] = t.y; u[4 * k + 2] = t.z; u[4 * k + 3] = t.w; }
+        const float2 t2 = *reinterpret_cast<const float2*>(link + 16);
+        u[16] = t2.x; u[17] = t2.y;
+    } else {
+        const double2* l2 = reinterpret_cast<const double2*>(link);
+#pragma unroll
+        for (int k = 0; k < 9; k++) { double2 t = l2[k]; u[2 * k] = t.x; u[2 * k + 1] = t.y; }
+    }
+    hop_dir_core<MU, SG, FWD>(acc, p, u);
 }
 
 // ---- the 4D-site-diagonal part of eq. 4: res[c] += c_diag psi(s) + coef psi(s -+ 1) ----------------
@@ -246,7 +257,7 @@ hop_kernel(const HopArgs<R> a) {
     const long long site = site0 + ls;
     if (ls >= a.GS || site >= a.V4h) return;
     const int BS = 12 * K;                                    // groups per (site, rhs) block
-    const long long blk = site * a.nrhs + r;
+    const long long blk = blk_index(site, r, a.nrhs, a.sg_shift);
 
     CV<V> acc[12];
 #pragma unroll
@@ -255,18 +266,18 @@ hop_kernel(const HopArgs<R> a) {
     if constexpr (HOP) {
         const int4* nb4 = reinterpret_cast<const int4*>(a.nbr[pi] + site * 8);
         const int4 n0 = __ldg(nb4), n1 = __ldg(nb4 + 1);
-        const G* in = a.in_hop[pi] + (size_t)r * BS + k;
-        const size_t sstride = (size_t)a.nrhs * BS;           // groups per site
+        const G* in = a.in_hop[pi] + k;
+        auto nb = [&](int n) -> const G* { return in + (size_t)blk_index(n, r, a.nrhs, a.sg_shift) * BS; };
         const R* u = s_link + ls * SITE;
         constexpr int SF = DAG ? +1 : -1;                     // projector sign on the forward hop
-        hop_dir<0, SF, true >(acc, in + (size_t)n0.x * sstride, K, u + 0 * SLOT);
-        hop_dir<0, -SF, false>(acc, in + (size_t)n0.y * sstride, K, u + 1 * SLOT);
-        hop_dir<1, SF, true >(acc, in + (size_t)n0.z * sstride, K, u + 2 * SLOT);
-        hop_dir<1, -SF, false>(acc, in + (size_t)n0.w * sstride, K, u + 3 * SLOT);
-        hop_dir<2, SF, true >(acc, in + (size_t)n1.x * sstride, K, u + 4 * SLOT);
-        hop_dir<2, -SF, false>(acc, in + (size_t)n1.y * sstride, K, u + 5 * SLOT);
-        hop_dir<3, SF, true >(acc, in + (size_t)n1.z * sstride, K, u + 6 * SLOT);
-        hop_dir<3, -SF, false>(acc, in + (size_t)n1.w * sstride, K, u + 7 * SLOT);
+        hop_dir<0, SF, true >(acc, nb(n0.x), K, u + 0 * SLOT);
+        hop_dir<0, -SF, false>(acc, nb(n0.y), K, u + 1 * SLOT);
+        hop_dir<1, SF, true >(acc, nb(n0.z), K, u + 2 * SLOT);
+        hop_dir<1, -SF, false>(acc, nb(n0.w), K, u + 3 * SLOT);
+        hop_dir<2, SF, true >(acc, nb(n1.x), K, u + 4 * SLOT);
+        hop_dir<2, -SF, false>(acc, nb(n1.y), K, u + 5 * SLOT);
+        hop_dir<3, SF, true >(acc, nb(n1.z), K, u + 6 * SLOT);
+        hop_dir<3, -SF, false>(acc, nb(n1.w), K, u + 7 * SLOT);
 #pragma unroll
         for (int c = 0; c < 12; c++) { acc[c].re = vmul(a.c_hop, acc[c].re); acc[c].im = vmul(a.c_hop, acc[c].im); }
     }

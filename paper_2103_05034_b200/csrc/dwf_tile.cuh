@@ -1,0 +1,238 @@
+// dwf_tile.cuh -- the tiled, persistent form of the stencil kernel (same arithmetic as dwf_hop.cuh).
+//
+// Used when the lattice is made of whole tiles of TS sites per parity (TS = 32: 4x4x2x2, TS = 16:
+// 4x2x2x2) and Ls is a compile-time size.  A work item is (tile, right-hand side, output parity);
+// thread = (site in tile, lane group k); persistent CTAs walk the items in launch order.
+//
+// Everything a tile needs that is reused or needs an index lookup arrives in shared memory by bulk
+// asynchronous copies (cp.async.bulk + mbarrier, SASS UBLKCP) issued one item ahead:
+//   * the tile's TS opposite-parity sites ("interior": the only spinor blocks used by more than one
+//     output site of the tile; one contiguous run of TS*BS groups thanks to the block order),
+//   * the tile's gathered links  [site][mu][U_mu(x) | U_mu(x-mu)]  pre-scaled by -1/2 (set_gauge),
+//   * the tile's neighbour table [site][8].
+// Halo blocks (each used by exactly one output site) and the self / axpby operands are read from
+// global memory.  res = sigma * hop' + self with hop' built from the scaled links (sigma = 1 for
+// D_DW, H_DW, D_PV: no scaling pass).  The self term is computed first, while the copies land.
+#pragma once
+#include "dwf_hop.cuh"
+
+namespace dwf {
+
+// ---- mbarrier + bulk async copy (TMA, 1-D) --------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    unsigned ok = 0;
+    while (!ok)
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared bulk copy, completion signalled on the mbarrier (bytes: multiple of 16, 16-byte aligned)
+__device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// gathered links of one site: 4 x (fwd 18 | bwd 18) reals + 16 bytes of padding, so that the four
+// sites of a warp read distinct banks (592 B fp32, 1168 B fp64)
+template <typename R> struct TileLinks { static constexpr int SITE = 4 * 36 + 16 / (int)sizeof(R); };
+
+template <typename R, int LS, int TS> struct TileGeom {
+    static constexpr int K = LS / Prec<R>::VL;
+    static constexpr int THREADS = TS * K;
+    static constexpr int MIN_CTAS = THREADS <= 128 ? 4 : THREADS <= 256 ? 2 : 1;
+    static constexpr int BS = 12 * K;
+    static constexpr unsigned INTERIOR_BYTES = TS * BS * 16;
+    static constexpr unsigned LINK_BYTES = TS * TileLinks<R>::SITE * sizeof(R);
+    static constexpr unsigned NBR_BYTES = TS * 8 * sizeof(int);
+    static constexpr unsigned SMALL_BYTES = LINK_BYTES + NBR_BYTES;
+    static constexpr unsigned SMEM_BYTES = 128 + INTERIOR_BYTES + 2 * SMALL_BYTES;
+};
+
+// load the 18 reals of one link from the gathered shared-memory layout; HALF = 0: U_mu(x), 1: U_mu(x-mu)
+template <int HALF>
+__device__ __forceinline__ void load_link(const float* pair, float (&u)[18]) {
+    if constexpr (HALF == 0) {
+        const float4* l4 = reinterpret_cast<const float4*>(pair);
+#pragma unroll
+        for (int j = 0; j < 4; j++) { const float4 t = l4[j]; u[4 * j] = t.x; u[4 * j + 1] = t.y; u[4 * j + 2] = t.z; u[4 * j + 3] = t.w; }
+        const float2 t2 = *reinterpret_cast<const float2*>(pair + 16);
+        u[16] = t2.x; u[17] = t2.y;
+    } else {                                                   // reals 18..35: 8-byte aligned head, then 16-byte aligned
+        const float2 t2 = *reinterpret_cast<const float2*>(pair + 18);
+        u[0] = t2.x; u[1] = t2.y;
+        const float4* l4 = reinterpret_cast<const float4*>(pair + 20);
+#pragma unroll
+        for (int j = 0; j < 4; j++) { const float4 t = l4[j]; u[2 + 4 * j] = t.x; u[3 + 4 * j] = t.y; u[4 + 4 * j] = t.z; u[5 + 4 * j] = t.w; }
+    }
+}
+template <int HALF>
+__device__ __forceinline__ void load_link(const double* pair, double (&u)[18]) {
+    const double2* l2 = reinterpret_cast<const double2*>(pair + 18 * HALF);
+#pragma unroll
+    for (int j = 0; j < 9; j++) { const double2 t = l2[j]; u[2 * j] = t.x; u[2 * j + 1] = t.y; }
+}
+
+// one direction: psi is a generic pointer (shared-memory interior block or global halo block)
+template <int MU, int SG, bool FWD, typename R, typename V, typename G>
+__device__ __forceinline__ void tile_dir(CV<V> (&acc)[12], const G* psi, const int cstride, const R* pair) {
+    CV<V> p[12];
+#pragma unroll
+    for (int c = 0; c < 12; c++) p[c] = unpack(ld_plain(psi + c * cstride));
+    R u[18];
+    load_link<FWD ? 0 : 1>(pair, u);
+    hop_dir_core<MU, SG, FWD>(acc, p, u);
+}
+
+template <typename R, int LS, int TS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY>
+__global__ void __launch_bounds__(TileGeom<R, LS, TS>::THREADS, TileGeom<R, LS, TS>::MIN_CTAS)
+hop_tile_kernel(const HopArgs<R> a) {
+    using V = typename Prec<R>::V;
+    using G = typename Prec<R>::G;
+    using TG = TileGeom<R, LS, TS>;
+    constexpr int K = TG::K, BS = TG::BS;
+    constexpr int SH = (TS == 32) ? 5 : 4;
+    constexpr int LSITE = TileLinks<R>::SITE;
+    extern __shared__ __align__(128) unsigned char smem[];
+    unsigned long long* bar_int = reinterpret_cast<unsigned long long*>(smem);          // interior landed
+    unsigned long long* bar_small = reinterpret_cast<unsigned long long*>(smem) + 1;    // [2]: links + nbr landed
+    const G* s_in = reinterpret_cast<const G*>(smem + 128);
+    unsigned char* s_small = smem + 128 + TG::INTERIOR_BYTES;
+
+    // work item w -> (tile gg, rhs r, parity slot pi): same order as the CTAs of the generic kernel
+    const unsigned rn = (unsigned)a.rn, cg = (unsigned)a.chunk_groups;     // item counts fit 32 bits (checked by the host)
+    auto decode = [&](long long w, long long& gg_out, int& r, int& pi) {
+        unsigned gg = (unsigned)w / rn;
+        r = a.r0 + (int)((unsigned)w - gg * rn);
+        pi = 0;
+        if (a.nslots == 2) {
+            const unsigned q = gg / (2 * cg);
+            const unsigned rem = gg - q * 2 * cg;
+            pi = rem >= cg;
+            gg = q * cg + (rem - pi * cg);
+        }
+        gg_out = gg;
+    };
+    auto issue_small = [&](long long w, int buf) {             // thread 0 only
+        long long gg; int r, pi; decode(w, gg, r, pi);
+        const int p = (a.parity0 + pi) & 1;
+        unsigned char* dst = s_small + buf * TG::SMALL_BYTES;
+        mbar_expect_tx(bar_small + buf, TG::SMALL_BYTES);
+        bulk_g2s(dst, a.glinks[p] + (size_t)gg * TS * LSITE, TG::LINK_BYTES, bar_small + buf);
+        bulk_g2s(dst + TG::LINK_BYTES, a.nbr[pi] + (size_t)gg * TS * 8, TG::NBR_BYTES, bar_small + buf);
+    };
+    auto issue_interior = [&](long long w) {                   // thread 0 only
+        long long gg; int r, pi; decode(w, gg, r, pi);
+        mbar_expect_tx(bar_int, TG::INTERIOR_BYTES);
+        bulk_g2s(smem + 128, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int);
+    };
+
+    long long w = blockIdx.x;
+    if (w >= a.nitems) return;
+    unsigned* done_count = reinterpret_cast<unsigned*>(smem + 64);  // warps that finished the hop phase of the current item
+    if (threadIdx.x == 0) {
+        mbar_init(bar_int, 1); mbar_init(bar_small, 1); mbar_init(bar_small + 1, 1);
+        mbar_fence_init();
+        *done_count = 0;
+        issue_small(w, 0); issue_interior(w);
+        if (w + gridDim.x < a.nitems) issue_small(w + gridDim.x, 1);
+    }
+    __syncthreads();
+    constexpr unsigned NWARPS = TG::THREADS / 32;
+
+    const int ls = threadIdx.x / K;                            // site within the tile
+    const int k = threadIdx.x - ls * K;
+
+    for (int it = 0; w < a.nitems; it++, w += gridDim.x) {
+        long long gg; int r, pi;
+        decode(w, gg, r, pi);
+        const long long wn = w + gridDim.x;
+        const int buf = it & 1;
+        const long long site = gg * TS + ls;
+        const long long blk = blk_index(site, r, a.nrhs, SH);
+
+        CV<V> acc[12];
+#pragma unroll
+        for (int c = 0; c < 12; c++) { acc[c].re = vzero(V()); acc[c].im = vzero(V()); }
+        const bool scaled = (a.sigma != R(1));
+        if constexpr (SELF) {                                  // global loads only: overlaps the copies in flight
+            self_term<DAG>(acc, a.in_self[pi] + (size_t)blk * BS, K, k, a.c_diag, a.mass);
+            if (HOP && scaled) {
+                const R inv = R(1) / a.sigma;
+#pragma unroll
+                for (int c = 0; c < 12; c++) { acc[c].re = vmul(inv, acc[c].re); acc[c].im = vmul(inv, acc[c].im); }
+            }
+        }
+        if constexpr (HOP) {
+            mbar_wait(bar_small + buf, (it >> 1) & 1);
+            const unsigned char* small = s_small + buf * TG::SMALL_BYTES;
+            const int4* nb4 = reinterpret_cast<const int4*>(small + TG::LINK_BYTES) + ls * 2;
+            const int4 n0 = nb4[0], n1 = nb4[1];
+            const R* u = reinterpret_cast<const R*>(small) + ls * LSITE;
+            const G* in = a.in_hop[pi] + k;
+            // neighbour block: inside the tile -> shared memory, else global memory
+            auto nb = [&](int n) -> const G* {
+                if ((long long)(n >> SH) == gg) return s_in + (n & (TS - 1)) * BS + k;
+                return in + (size_t)blk_index(n, r, a.nrhs, SH) * BS;
+            };
+            const G* q0 = nb(n0.x); const G* q1 = nb(n0.y); const G* q2 = nb(n0.z); const G* q3 = nb(n0.w);
+            const G* q4 = nb(n1.x); const G* q5 = nb(n1.y); const G* q6 = nb(n1.z); const G* q7 = nb(n1.w);
+            constexpr int SF = DAG ? +1 : -1;                  // projector sign on the forward hop
+            mbar_wait(bar_int, it & 1);
+            tile_dir<0, SF, true >(acc, q0, K, u + 0 * 36);
+            tile_dir<0, -SF, false>(acc, q1, K, u + 0 * 36);
+            tile_dir<1, SF, true >(acc, q2, K, u + 1 * 36);
+            tile_dir<1, -SF, false>(acc, q3, K, u + 1 * 36);
+            tile_dir<2, SF, true >(acc, q4, K, u + 2 * 36);
+            tile_dir<2, -SF, false>(acc, q5, K, u + 2 * 36);
+            tile_dir<3, SF, true >(acc, q6, K, u + 3 * 36);
+            tile_dir<3, -SF, false>(acc, q7, K, u + 3 * 36);
+            // The last warp to finish the hop phase of this item refills the buffers: the interior with item
+            // it+1, this small buffer with item it+2 (nobody waits: the arrival is awaited through the mbarriers).
+            __syncwarp();
+            if ((threadIdx.x & 31) == 0) {
+                const unsigned prev = atomicAdd(done_count, 1u);
+                if (prev == (unsigned)(it + 1) * NWARPS - 1) {
+                    if (wn < a.nitems) issue_interior(wn);
+                    if (wn + gridDim.x < a.nitems) issue_small(wn + gridDim.x, buf);
+                }
+            }
+            if (scaled) {
+#pragma unroll
+                for (int c = 0; c < 12; c++) { acc[c].re = vmul(a.sigma, acc[c].re); acc[c].im = vmul(a.sigma, acc[c].im); }
+            }
+        }
+        int ko = k;
+        if constexpr (G5) {
+            ko = K - 1 - k;
+#pragma unroll
+            for (int c = 0; c < 12; c++) {
+                acc[c].re = vswap(acc[c].re); acc[c].im = vswap(acc[c].im);
+                if (c >= 6) { acc[c].re = vneg(acc[c].re); acc[c].im = vneg(acc[c].im); }
+            }
+        }
+        const size_t obase = (size_t)blk * BS + ko;
+        if constexpr (AXPBY) {
+            const G* y = a.y[pi] + obase;
+            const G* z = a.z[pi] + obase;
+#pragma unroll
+            for (int c = 0; c < 12; c++) {
+                const CV<V> yy = unpack(ldg_nc(y + c * K));
+                const CV<V> zz = unpack(ld_plain(z + c * K));
+                acc[c].re = vfma(a.ax_c, zz.re, vfma(a.ax_b, yy.re, vmul(a.ax_a, acc[c].re)));
+                acc[c].im = vfma(a.ax_c, zz.im, vfma(a.ax_b, yy.im, vmul(a.ax_a, acc[c].im)));
+            }
+        }
+        G* o = a.out[pi] + obase;
+#pragma unroll
+        for (int c = 0; c < 12; c++) o[c * K] = pack(acc[c]);
+    }
+}
+
+}  // namespace dwf

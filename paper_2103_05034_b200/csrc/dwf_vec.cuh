@@ -60,4 +60,12 @@ __device__ __forceinline__ double2 ldg_nc(const double2* p) { return __ldg(p); }
 __device__ __forceinline__ float4 ld_plain(const float4* p) { return *p; }
 __device__ __forceinline__ double2 ld_plain(const double2* p) { return *p; }
 
+// Block index of (site, rhs) in a half field: sites come in groups of 2^sg_shift
+// (one tile of the native site order); a group's blocks are ordered [rhs][site in group], so that the
+// tile of one right-hand side is one contiguous run (a single bulk copy).
+__device__ __forceinline__ long long blk_index(long long site, int r, int nrhs, int sg_shift) {
+    const long long grp = site >> sg_shift;
+    return ((grp * nrhs + r) << sg_shift) + (site - (grp << sg_shift));
+}
+
 }  // namespace dwf
