@@ -16,6 +16,16 @@
 #pragma once
 #include "dwf_hop.cuh"
 
+#ifndef DWF_INT_STAGES
+#define DWF_INT_STAGES 1     // shared-memory buffers for the tile interior (2: warps may run one item ahead)
+#endif
+#ifndef DWF_MINCTAS128
+#define DWF_MINCTAS128 4
+#endif
+#ifndef DWF_MINCTAS256
+#define DWF_MINCTAS256 2
+#endif
+
 namespace dwf {
 
 // ---- mbarrier + bulk async copy (TMA, 1-D) --------------------------------------------------------
@@ -46,13 +56,14 @@ template <typename R> struct TileLinks { static constexpr int SITE = 4 * 36 + 16
 template <typename R, int LS, int TS> struct TileGeom {
     static constexpr int K = LS / Prec<R>::VL;
     static constexpr int THREADS = TS * K;
-    static constexpr int MIN_CTAS = THREADS <= 128 ? 4 : THREADS <= 256 ? 2 : 1;
+    static constexpr int MIN_CTAS = THREADS <= 128 ? DWF_MINCTAS128 : THREADS <= 256 ? DWF_MINCTAS256 : 1;
+    static constexpr int NSTI = DWF_INT_STAGES;
     static constexpr int BS = 12 * K;
     static constexpr unsigned INTERIOR_BYTES = TS * BS * 16;
     static constexpr unsigned LINK_BYTES = TS * TileLinks<R>::SITE * sizeof(R);
     static constexpr unsigned NBR_BYTES = TS * 8 * sizeof(int);
     static constexpr unsigned SMALL_BYTES = LINK_BYTES + NBR_BYTES;
-    static constexpr unsigned SMEM_BYTES = 128 + INTERIOR_BYTES + 2 * SMALL_BYTES;
+    static constexpr unsigned SMEM_BYTES = 128 + NSTI * INTERIOR_BYTES + 2 * SMALL_BYTES;
 };
 
 // load the 18 reals of one link from the gathered shared-memory layout; HALF = 0: U_mu(x), 1: U_mu(x-mu)
@@ -100,10 +111,10 @@ hop_tile_kernel(const HopArgs<R> a) {
     constexpr int SH = (TS == 32) ? 5 : 4;
     constexpr int LSITE = TileLinks<R>::SITE;
     extern __shared__ __align__(128) unsigned char smem[];
-    unsigned long long* bar_int = reinterpret_cast<unsigned long long*>(smem);          // interior landed
-    unsigned long long* bar_small = reinterpret_cast<unsigned long long*>(smem) + 1;    // [2]: links + nbr landed
-    const G* s_in = reinterpret_cast<const G*>(smem + 128);
-    unsigned char* s_small = smem + 128 + TG::INTERIOR_BYTES;
+    constexpr int NSTI = TG::NSTI;
+    unsigned long long* bar_int = reinterpret_cast<unsigned long long*>(smem);          // [NSTI]: interior landed
+    unsigned long long* bar_small = reinterpret_cast<unsigned long long*>(smem) + 2;    // [2]: links + nbr landed
+    unsigned char* s_small = smem + 128 + NSTI * TG::INTERIOR_BYTES;
 
     // work item w -> (tile gg, rhs r, parity slot pi): same order as the CTAs of the generic kernel
     const unsigned rn = (unsigned)a.rn, cg = (unsigned)a.chunk_groups;     // item counts fit 32 bits (checked by the host)
@@ -127,21 +138,21 @@ hop_tile_kernel(const HopArgs<R> a) {
         bulk_g2s(dst, a.glinks[p] + (size_t)gg * TS * LSITE, TG::LINK_BYTES, bar_small + buf);
         bulk_g2s(dst + TG::LINK_BYTES, a.nbr[pi] + (size_t)gg * TS * 8, TG::NBR_BYTES, bar_small + buf);
     };
-    auto issue_interior = [&](long long w) {                   // thread 0 only
+    auto issue_interior = [&](long long w, int ib) {           // thread 0 only
         long long gg; int r, pi; decode(w, gg, r, pi);
-        mbar_expect_tx(bar_int, TG::INTERIOR_BYTES);
-        bulk_g2s(smem + 128, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int);
+        mbar_expect_tx(bar_int + ib, TG::INTERIOR_BYTES);
+        bulk_g2s(smem + 128 + ib * TG::INTERIOR_BYTES, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int + ib);
     };
 
     long long w = blockIdx.x;
     if (w >= a.nitems) return;
-    unsigned* done_count = reinterpret_cast<unsigned*>(smem + 64);  // warps that finished the hop phase of the current item
+    unsigned* done_count = reinterpret_cast<unsigned*>(smem + 64);  // [2]: warps that finished the hop phase of even / odd items
     if (threadIdx.x == 0) {
-        mbar_init(bar_int, 1); mbar_init(bar_small, 1); mbar_init(bar_small + 1, 1);
+        mbar_init(bar_int, 1); mbar_init(bar_int + 1, 1); mbar_init(bar_small, 1); mbar_init(bar_small + 1, 1);
         mbar_fence_init();
-        *done_count = 0;
-        issue_small(w, 0); issue_interior(w);
-        if (w + gridDim.x < a.nitems) issue_small(w + gridDim.x, 1);
+        done_count[0] = 0; done_count[1] = 0;
+        issue_small(w, 0); issue_interior(w, 0);
+        if (w + gridDim.x < a.nitems) { issue_small(w + gridDim.x, 1); if (NSTI == 2) issue_interior(w + gridDim.x, 1); }
     }
     __syncthreads();
     constexpr unsigned NWARPS = TG::THREADS / 32;
@@ -175,6 +186,8 @@ hop_tile_kernel(const HopArgs<R> a) {
             const int4* nb4 = reinterpret_cast<const int4*>(small + TG::LINK_BYTES) + ls * 2;
             const int4 n0 = nb4[0], n1 = nb4[1];
             const R* u = reinterpret_cast<const R*>(small) + ls * LSITE;
+            const int ib = (NSTI == 2) ? buf : 0;
+            const G* s_in = reinterpret_cast<const G*>(smem + 128 + ib * TG::INTERIOR_BYTES);
             const G* in = a.in_hop[pi] + k;
             // neighbour block: inside the tile -> shared memory, else global memory
             auto nb = [&](int n) -> const G* {
@@ -184,7 +197,7 @@ hop_tile_kernel(const HopArgs<R> a) {
             const G* q0 = nb(n0.x); const G* q1 = nb(n0.y); const G* q2 = nb(n0.z); const G* q3 = nb(n0.w);
             const G* q4 = nb(n1.x); const G* q5 = nb(n1.y); const G* q6 = nb(n1.z); const G* q7 = nb(n1.w);
             constexpr int SF = DAG ? +1 : -1;                  // projector sign on the forward hop
-            mbar_wait(bar_int, it & 1);
+            mbar_wait(bar_int + ib, (NSTI == 2) ? (it >> 1) & 1 : it & 1);
             tile_dir<0, SF, true >(acc, q0, K, u + 0 * 36);
             tile_dir<0, -SF, false>(acc, q1, K, u + 0 * 36);
             tile_dir<1, SF, true >(acc, q2, K, u + 1 * 36);
@@ -197,10 +210,10 @@ hop_tile_kernel(const HopArgs<R> a) {
             // it+1, this small buffer with item it+2 (nobody waits: the arrival is awaited through the mbarriers).
             __syncwarp();
             if ((threadIdx.x & 31) == 0) {
-                const unsigned prev = atomicAdd(done_count, 1u);
-                if (prev == (unsigned)(it + 1) * NWARPS - 1) {
-                    if (wn < a.nitems) issue_interior(wn);
-                    if (wn + gridDim.x < a.nitems) issue_small(wn + gridDim.x, buf);
+                const unsigned prev = atomicAdd(done_count + buf, 1u);
+                if (prev == (unsigned)((it >> 1) + 1) * NWARPS - 1) {
+                    if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);
+                    if (wn + gridDim.x < a.nitems) { issue_small(wn + gridDim.x, buf); if (NSTI == 2) issue_interior(wn + gridDim.x, buf); }
                 }
             }
             if (scaled) {
