@@ -251,7 +251,7 @@ extern "C" int dwf_export(dwf_handle h, const void* native, void* canonical, int
 // ------------------------------------------------------------------------------------------------
 // Stencil dispatch
 // ------------------------------------------------------------------------------------------------
-enum HopMode { HM_HOP, HM_HOP_SELF, HM_HOP_SELF_G5, HM_HOP_SELF_G5_AXPBY, HM_SELF };
+enum HopMode { HM_HOP, HM_HOP_SELF, HM_HOP_SELF_G5, HM_HOP_SELF_G5_AXPBY, HM_SELF, HM_HOP_MOOINV /* tiled only */ };
 
 struct HopCall {            // precision-independent description of one launch
     int mode; bool dag;
@@ -291,10 +291,15 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.glinks[0] = (const R*)h->glinks;
     a.glinks[1] = (const R*)((const char*)h->glinks + (size_t)h->V4h * lsite);
     a.sigma = (R)(-2.0 * k.c_hop);                                             // links carry the factor -1/2
+    {
+        const double kappa = 1.0 / (5.0 - h->M5);
+        a.moo_kappa = (R)kappa; a.moo_v0scale = (R)(kappa / (1.0 + k.mass * std::pow(kappa, (double)h->Ls)));
+    }
+    if (k.mode == HM_HOP_MOOINV && !TS) FAIL(h, DWF_EINVAL, "fused hop + M_oo^-1 needs the tiled kernel");
 #define HOPK(LS, DAG, HOP, SELF, G5, AX) hop_kernel<R, LS, DAG, HOP, SELF, G5, AX><<<grid, HOP_THREADS, 0, st>>>(a)
-#define TILEK(LS, TSV, DAG, SELF, G5, AX) do { \
+#define TILEK(LS, TSV, DAG, SELF, G5, AX, MOO) do { \
         using TG = TileGeom<R, LS, TSV>; \
-        auto kern = hop_tile_kernel<R, LS, TSV, DAG, true, SELF, G5, AX>; \
+        auto kern = hop_tile_kernel<R, LS, TSV, DAG, true, SELF, G5, AX, MOO>; \
         cudaError_t e_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TG::SMEM_BYTES); \
         if (e_ != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e_)); \
         const long long ctas = std::min<long long>(a.nitems, (long long)h->sm_count * TG::MIN_CTAS); \
@@ -310,10 +315,11 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     }
 #define TILEM(LS, TSV) \
     switch (k.mode) { \
-        case HM_HOP:               if (k.dag) TILEK(LS, TSV, true, false, false, false); else TILEK(LS, TSV, false, false, false, false); break; \
-        case HM_HOP_SELF:          if (k.dag) TILEK(LS, TSV, true, true, false, false);  else TILEK(LS, TSV, false, true, false, false); break; \
-        case HM_HOP_SELF_G5:       TILEK(LS, TSV, false, true, true, false); break; \
-        case HM_HOP_SELF_G5_AXPBY: TILEK(LS, TSV, false, true, true, true); break; \
+        case HM_HOP:               if (k.dag) TILEK(LS, TSV, true, false, false, false, false); else TILEK(LS, TSV, false, false, false, false, false); break; \
+        case HM_HOP_MOOINV:        if (k.dag) TILEK(LS, TSV, true, false, false, false, true); else TILEK(LS, TSV, false, false, false, false, true); break; \
+        case HM_HOP_SELF:          if (k.dag) TILEK(LS, TSV, true, true, false, false, false);  else TILEK(LS, TSV, false, true, false, false, false); break; \
+        case HM_HOP_SELF_G5:       TILEK(LS, TSV, false, true, true, false, false); break; \
+        case HM_HOP_SELF_G5_AXPBY: TILEK(LS, TSV, false, true, true, true, false); break; \
         default: FAIL(h, DWF_EINVAL, "bad hop mode"); \
     }
     // Right-hand sides are processed in chunks (one launch each) so that the working set of a chunk keeps
@@ -381,11 +387,13 @@ static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, co
 // Schur operator on even half fields:  tmp_o = M_oo^-1 Dhop_oe in ;
 // out = M_ee in - 1/4 Dhop_eo tmp_o     [M_eo = M_oe = -1/2 Dhop].  dag: every factor adjoint.
 static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs) {
+    // K1: tmp_o = M_oo^-1 Dhop_oe in -- one launch when the tiled kernel applies (M_oo^-1 fused as its epilogue)
+    const bool fused = h->glinks && h->tile_sites && (h->Ls == 16 || h->Ls == 24) && !getenv("DWF_NO_FUSE_MOOINV");
     HopCall k1{};
-    k1.mode = HM_HOP; k1.dag = dag; k1.nslots = 1; k1.parity0 = 1; k1.nrhs = nrhs;
+    k1.mode = fused ? HM_HOP_MOOINV : HM_HOP; k1.dag = dag; k1.nslots = 1; k1.parity0 = 1; k1.nrhs = nrhs;
     k1.in_hop[0] = in; k1.out[0] = tmp; k1.c_hop = 1.0; k1.mass = h->mass;
     if (int rc = launch_hop(h, k1)) return rc;
-    if (int rc = launch_mooinv(h, tmp, tmp, nrhs, h->mass, dag)) return rc;
+    if (!fused) { if (int rc = launch_mooinv(h, tmp, tmp, nrhs, h->mass, dag)) return rc; }
     HopCall k2{};
     k2.mode = HM_HOP_SELF; k2.dag = dag; k2.nslots = 1; k2.parity0 = 0; k2.nrhs = nrhs;
     k2.in_hop[0] = tmp; k2.in_self[0] = in; k2.out[0] = out; k2.c_hop = -0.25; k2.mass = h->mass;

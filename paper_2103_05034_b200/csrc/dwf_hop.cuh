@@ -41,6 +41,7 @@ template <typename R> struct HopArgs {
     // tiled kernel only (dwf_tile.cuh):
     const R* glinks[2];    // [p] gathered links of parity-p sites: [site][mu][fwd 18 | bwd 18] x (-1/2), 16 B pad per site
     R sigma;               // res = sigma * hop' + self  with hop' built from the (-1/2)-scaled links
+    R moo_kappa, moo_v0scale;   // fused M_oo^-1 epilogue: 1/(5-M5), kappa / (1 + m kappa^Ls)
     long long nitems;      // work items (tile, rhs, parity slot) of this launch
     long long ngroups;     // ceil(V4h / G)
     long long chunk_groups;

@@ -22,6 +22,9 @@
 #ifndef DWF_MINCTAS128
 #define DWF_MINCTAS128 4
 #endif
+#ifndef DWF_MINCTAS192
+#define DWF_MINCTAS192 2
+#endif
 #ifndef DWF_MINCTAS256
 #define DWF_MINCTAS256 2
 #endif
@@ -56,14 +59,17 @@ template <typename R> struct TileLinks { static constexpr int SITE = 4 * 36 + 16
 template <typename R, int LS, int TS> struct TileGeom {
     static constexpr int K = LS / Prec<R>::VL;
     static constexpr int THREADS = TS * K;
-    static constexpr int MIN_CTAS = THREADS <= 128 ? DWF_MINCTAS128 : THREADS <= 256 ? DWF_MINCTAS256 : 1;
+    static constexpr int MIN_CTAS = THREADS <= 128 ? DWF_MINCTAS128 : THREADS <= 192 ? DWF_MINCTAS192 : THREADS <= 256 ? DWF_MINCTAS256 : 1;
     static constexpr int NSTI = DWF_INT_STAGES;
     static constexpr int BS = 12 * K;
     static constexpr unsigned INTERIOR_BYTES = TS * BS * 16;
     static constexpr unsigned LINK_BYTES = TS * TileLinks<R>::SITE * sizeof(R);
     static constexpr unsigned NBR_BYTES = TS * 8 * sizeof(int);
     static constexpr unsigned SMALL_BYTES = LINK_BYTES + NBR_BYTES;
-    static constexpr unsigned SMEM_BYTES = 128 + NSTI * INTERIOR_BYTES + 2 * SMALL_BYTES;
+    // the fused M_oo^-1 epilogue transposes the tile through the interior buffer with rows padded by one group
+    static constexpr unsigned TRANS_BYTES = TS * 12 * (K + 1) * 16;
+    static constexpr unsigned INT_STRIDE = INTERIOR_BYTES > TRANS_BYTES ? INTERIOR_BYTES : TRANS_BYTES;
+    static constexpr unsigned SMEM_BYTES = 128 + NSTI * INT_STRIDE + 2 * SMALL_BYTES;
 };
 
 // load the 18 reals of one link from the gathered shared-memory layout; HALF = 0: U_mu(x), 1: U_mu(x-mu)
@@ -101,9 +107,10 @@ __device__ __forceinline__ void tile_dir(CV<V> (&acc)[12], const G* psi, const i
     hop_dir_core<MU, SG, FWD>(acc, p, u);
 }
 
-template <typename R, int LS, int TS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY>
+template <typename R, int LS, int TS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY, bool MOO = false>
 __global__ void __launch_bounds__(TileGeom<R, LS, TS>::THREADS, TileGeom<R, LS, TS>::MIN_CTAS)
 hop_tile_kernel(const HopArgs<R> a) {
+    static_assert(!MOO || (HOP && !SELF && !G5 && !AXPBY && TileGeom<R, LS, TS>::NSTI == 1), "fused M_oo^-1 follows a bare hop");
     using V = typename Prec<R>::V;
     using G = typename Prec<R>::G;
     using TG = TileGeom<R, LS, TS>;
@@ -114,7 +121,7 @@ hop_tile_kernel(const HopArgs<R> a) {
     constexpr int NSTI = TG::NSTI;
     unsigned long long* bar_int = reinterpret_cast<unsigned long long*>(smem);          // [NSTI]: interior landed
     unsigned long long* bar_small = reinterpret_cast<unsigned long long*>(smem) + 2;    // [2]: links + nbr landed
-    unsigned char* s_small = smem + 128 + NSTI * TG::INTERIOR_BYTES;
+    unsigned char* s_small = smem + 128 + NSTI * TG::INT_STRIDE;
 
     // work item w -> (tile gg, rhs r, parity slot pi): same order as the CTAs of the generic kernel
     const unsigned rn = (unsigned)a.rn, cg = (unsigned)a.chunk_groups;     // item counts fit 32 bits (checked by the host)
@@ -141,7 +148,7 @@ hop_tile_kernel(const HopArgs<R> a) {
     auto issue_interior = [&](long long w, int ib) {           // thread 0 only
         long long gg; int r, pi; decode(w, gg, r, pi);
         mbar_expect_tx(bar_int + ib, TG::INTERIOR_BYTES);
-        bulk_g2s(smem + 128 + ib * TG::INTERIOR_BYTES, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int + ib);
+        bulk_g2s(smem + 128 + ib * TG::INT_STRIDE, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int + ib);
     };
 
     long long w = blockIdx.x;
@@ -187,7 +194,7 @@ hop_tile_kernel(const HopArgs<R> a) {
             const int4 n0 = nb4[0], n1 = nb4[1];
             const R* u = reinterpret_cast<const R*>(small) + ls * LSITE;
             const int ib = (NSTI == 2) ? buf : 0;
-            const G* s_in = reinterpret_cast<const G*>(smem + 128 + ib * TG::INTERIOR_BYTES);
+            const G* s_in = reinterpret_cast<const G*>(smem + 128 + ib * TG::INT_STRIDE);
             const G* in = a.in_hop[pi] + k;
             // neighbour block: inside the tile -> shared memory, else global memory
             auto nb = [&](int n) -> const G* {
@@ -206,19 +213,69 @@ hop_tile_kernel(const HopArgs<R> a) {
             tile_dir<2, -SF, false>(acc, q5, K, u + 2 * 36);
             tile_dir<3, SF, true >(acc, q6, K, u + 3 * 36);
             tile_dir<3, -SF, false>(acc, q7, K, u + 3 * 36);
-            // The last warp to finish the hop phase of this item refills the buffers: the interior with item
-            // it+1, this small buffer with item it+2 (nobody waits: the arrival is awaited through the mbarriers).
-            __syncwarp();
-            if ((threadIdx.x & 31) == 0) {
-                const unsigned prev = atomicAdd(done_count + buf, 1u);
-                if (prev == (unsigned)((it >> 1) + 1) * NWARPS - 1) {
-                    if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);
-                    if (wn + gridDim.x < a.nitems) { issue_small(wn + gridDim.x, buf); if (NSTI == 2) issue_interior(wn + gridDim.x, buf); }
+            // The last warp to finish with the shared-memory buffers of this item refills them: the interior with
+            // item it+1, this small buffer with item it+2 (nobody waits: arrival is awaited through the mbarriers).
+            auto release_buffers = [&]() {
+                __syncwarp();
+                if ((threadIdx.x & 31) == 0) {
+                    const unsigned prev = atomicAdd(done_count + buf, 1u);
+                    if (prev == (unsigned)((it >> 1) + 1) * NWARPS - 1) {
+                        if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);
+                        if (wn + gridDim.x < a.nitems) { issue_small(wn + gridDim.x, buf); if (NSTI == 2) issue_interior(wn + gridDim.x, buf); }
+                    }
                 }
-            }
+            };
+            if constexpr (!MOO) release_buffers();
             if (scaled) {
 #pragma unroll
                 for (int c = 0; c < 12; c++) { acc[c].re = vmul(a.sigma, acc[c].re); acc[c].im = vmul(a.sigma, acc[c].im); }
+            }
+            if constexpr (MOO) {
+                // out = M_oo^-1 res (closed form of DESIGN.md sec. 5.4), fused: the tile is transposed through the
+                // interior buffer (rows = (site, component), padded by one group against bank conflicts), then one
+                // thread per row walks s in registers and stores the row (contiguous in the output block).
+                constexpr int VL = Prec<R>::VL;
+                G* s_t = reinterpret_cast<G*>(smem + 128);
+                __syncthreads();                               // every warp is done reading the interior
+#pragma unroll
+                for (int c = 0; c < 12; c++) s_t[(ls * 12 + c) * (K + 1) + k] = pack(acc[c]);
+                __syncthreads();
+                const R kappa = a.moo_kappa, v0scale = a.moo_v0scale, mass = a.mass;
+                G* obase_t = a.out[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS;   // the tile's blocks are one run
+                for (int row = threadIdx.x; row < TS * 12; row += TG::THREADS) {
+                    const int c = row % 12;
+                    const bool down = DAG ? (c >= 6) : (c < 6);
+                    R bre[LS], bim[LS];
+#pragma unroll
+                    for (int kk = 0; kk < K; kk++) {
+                        const G g = s_t[row * (K + 1) + (down ? kk : K - 1 - kk)];
+                        if constexpr (VL == 2) {
+                            bre[2 * kk] = down ? g.x : g.y; bre[2 * kk + 1] = down ? g.y : g.x;
+                            bim[2 * kk] = down ? g.z : g.w; bim[2 * kk + 1] = down ? g.w : g.z;
+                        } else { bre[kk] = g.x; bim[kk] = g.y; }
+                    }
+                    const R b0re = bre[0], b0im = bim[0];
+                    bre[0] = R(0); bim[0] = R(0);
+#pragma unroll
+                    for (int j = 1; j < LS; j++) { bre[j] = kappa * (bre[j] + bre[j - 1]); bim[j] = kappa * (bim[j] + bim[j - 1]); }
+                    const R v0re = v0scale * (b0re - mass * bre[LS - 1]);
+                    const R v0im = v0scale * (b0im - mass * bim[LS - 1]);
+                    R pw = R(1);
+#pragma unroll
+                    for (int j = 0; j < LS; j++) { bre[j] = fma(pw, v0re, bre[j]); bim[j] = fma(pw, v0im, bim[j]); pw *= kappa; }
+                    G* orow = obase_t + (size_t)row * K;
+#pragma unroll
+                    for (int kk = 0; kk < K; kk++) {
+                        G g;
+                        if constexpr (VL == 2) {
+                            g.x = down ? bre[2 * kk] : bre[2 * kk + 1]; g.y = down ? bre[2 * kk + 1] : bre[2 * kk];
+                            g.z = down ? bim[2 * kk] : bim[2 * kk + 1]; g.w = down ? bim[2 * kk + 1] : bim[2 * kk];
+                        } else { g.x = bre[kk]; g.y = bim[kk]; }
+                        orow[down ? kk : K - 1 - kk] = g;
+                    }
+                }
+                release_buffers();                             // the solver's reads of the buffer are complete (values consumed)
+                continue;
             }
         }
         int ko = k;
