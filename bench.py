@@ -161,6 +161,23 @@ def run_only(args, dev):
     name = args.only
     if name.endswith("_48"):
         return run_only_config4(args, dev)
+    if name == "cg_8":                                       # BASELINE.json configs[1]: 8^4 x 16, 50 rb-CG iterations (launch-bound size)
+        L8 = (8, 8, 8, 8)
+        d = Dwf(L8, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)
+        d.set_gauge(torch.from_numpy(gen.gauge_random(L8, 1001)).to(d.cdtype).to(dev))
+        d.set_workspace(1)
+        g = torch.Generator(device=dev); g.manual_seed(2001)
+        b = d.field(1, half=True).normal_(generator=g); x = d.field(1, half=True, zero=True)
+        for _ in range(3):
+            x.zero_(); d.cg_schur(b, x, 50)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            x.zero_(); d.cg_schur(b, x, 50)
+        torch.cuda.synchronize()
+        ms = (time.perf_counter() - t0) * 1e3 / args.steps
+        print(json.dumps({"only": name, "prec": args.prec, "iters": 50, "ms": round(ms, 3), "iterations/s": round(51 / ms * 1e3, 1)}), flush=True)
+        return
     d = Dwf(L, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)
     d.set_gauge(torch.from_numpy(gen.gauge_random(L, 1002)).to(d.cdtype).to(dev))
     g = torch.Generator(device=dev); g.manual_seed(2002)
