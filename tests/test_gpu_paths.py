@@ -1,0 +1,64 @@
+"""GPU: the alternative kernel paths of libdwf agree with each other (every path is also compared with the
+oracle in test_gpu_parity.py / test_gpu_fullsize.py through whichever path is the default).
+
+  * tiled persistent stencil (dwf_tile.cuh)  vs  generic stencil (dwf_hop.cuh)      DWF_NO_TILE=1
+  * Schur K1 with the fused M_oo^-1 epilogue vs  separate mooinv_kernel            DWF_NO_FUSE_MOOINV=1
+  * CG enqueued on the stream                vs  CG captured into a CUDA graph     DWF_CG_GRAPH=1
+"""
+import numpy as np
+import pytest
+
+import dwf_inputs as gen
+from gpu_util import M5, Rig, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+from paper_2103_05034_b200 import DWF_DAGGER, DWF_DDW, DWF_DHOP, DWF_HDW, DWF_SCHUR_EO  # noqa: E402
+
+
+@pytest.mark.parametrize("prec,L,Ls,nrhs", [("f32", (8, 8, 4, 4), 16, 3), ("f64", (8, 4, 4, 4), 16, 2), ("f32", (8, 4, 4, 8), 24, 2)])
+def test_tiled_vs_generic(oracle, monkeypatch, prec, L, Ls, nrhs):
+    mass = 0.03
+    tol = 1e-12 if prec == "f64" else 2e-6
+    psi = None
+    outs = {}
+    for tag, env in (("tiled", None), ("generic", "1")):
+        if env:
+            monkeypatch.setenv("DWF_NO_TILE", env)
+        rig = Rig(L, Ls, prec, mass, seed_U=31, ws_nrhs=nrhs)
+        if psi is None:
+            psi = rig.spinor(nrhs, 32)
+        pe = gen.keep_parity(psi, L, 0)
+        outs[tag] = [rig.apply(DWF_DHOP, psi), rig.apply(DWF_DDW, psi), rig.apply(DWF_HDW, psi), rig.apply(DWF_DDW | DWF_DAGGER, psi),
+                     rig.apply(DWF_SCHUR_EO, pe, half=True), rig.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True)]
+        cheb = rig.d.field(nrhs)
+        rig.d.chebyshev(5, 0.01, 70.0, rig.native(psi), cheb, nrhs)
+        outs[tag].append(rig.canonical(cheb, nrhs))
+    for a, b in zip(outs["tiled"], outs["generic"]):
+        assert rel_l2(a, b) < tol
+    # and one of them against the oracle, so that the pair is anchored
+    assert rel_l2(outs["generic"][1], oracle.ddw(rig.U, psi, M5, mass)) < (1e-12 if prec == "f64" else 1e-5)
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_fused_mooinv_vs_separate(monkeypatch, prec):
+    L, Ls, mass, nrhs = (8, 4, 8, 4), 16, 0.01, 2
+    rig = Rig(L, Ls, prec, mass, seed_U=41, ws_nrhs=nrhs)
+    pe = gen.keep_parity(rig.spinor(nrhs, 42), L, 0)
+    fused = [rig.apply(DWF_SCHUR_EO, pe, half=True), rig.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True)]
+    monkeypatch.setenv("DWF_NO_FUSE_MOOINV", "1")
+    sep = [rig.apply(DWF_SCHUR_EO, pe, half=True), rig.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True)]
+    for a, b in zip(fused, sep):
+        assert np.array_equal(a, b)                   # same arithmetic in the same order: bit identical
+
+
+def test_cg_graph_vs_stream(monkeypatch):
+    L, Ls, mass = (8, 8, 8, 8), 16, 0.01
+    rig = Rig(L, Ls, "f32", mass, seed_U=1001, ws_nrhs=1)
+    b = rig.native(gen.keep_parity(rig.spinor(1, 2001), L, 0), 0)
+    x1 = rig.d.field(1, half=True, zero=True)
+    h1 = rig.d.cg_schur(b, x1, 20)
+    monkeypatch.setenv("DWF_CG_GRAPH", "1")
+    x2 = rig.d.field(1, half=True, zero=True)
+    h2 = rig.d.cg_schur(b, x2, 20)
+    assert h1 == h2 and bool((x1 == x2).all())        # deterministic reductions: bit identical
