@@ -34,6 +34,10 @@ V5 = L[0] * L[1] * L[2] * L[3] * LS
 FLOP_PER_SITE = 1320.0
 CHEB_ORDER, CHEB_NVEC, CHEB_LO, CHEB_HI = 64, 24, 0.01, 70.0
 CG_ITERS = 20
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (ncu --set full; average of the two
+# epilogue variants), filled in from the capture summarised in NCU_TRAFFIC_SOURCE
+NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_SOURCE = "profiles/r1_10_cheb_tile.md"
 WORKLOAD = "16^3x32xLs16 fp32: D_hop/D_DW/H_DW/D_PV (nrhs 1,12,48) + Schur(4) + BLAS-1 + order-64 Chebyshev(24) + 20 rb-CG it"
 
 
@@ -392,20 +396,21 @@ def main():
     for name in ("a1_import_export", "schur_nrhs4", "blas1_nrhs12"):
         detail[name] = {"ms": round(avg_ms(name), 4)}
 
-    # dominant kernel = hop_kernel inside dwf_chebyshev: 2*order launches per call; its average launch duration
-    # = event-bracketed call time / launches; algorithmic bytes per launch = cheb_bytes / (2*order).
-    n_launch = 2 * CHEB_ORDER
-    ach = cheb_bytes(CHEB_ORDER, CHEB_NVEC) / n_launch / (t_cheb / n_launch) / 1e6
-    roofline = {"bound": "hbm", "kernel": "dwf::hop_kernel<float,...> (H_DW and H_DW+axpby epilogues, nrhs=24, inside dwf_chebyshev)",
+    # dominant kernel = dwf::hop_tile_kernel inside dwf_chebyshev (H_DW and H_DW + three-term-recurrence epilogues,
+    # one launch per right-hand side and apply).  Its average launch duration = CUDA-event-bracketed call time
+    # on the launching stream / launches of the call; algorithmic bytes per launch = cheb_bytes / launches.
+    lc0 = d.launch_count()
+    d.chebyshev(CHEB_ORDER, CHEB_LO, CHEB_HI, xc, yc, CHEB_NVEC)
+    torch.cuda.synchronize()
+    n_launch = d.launch_count() - lc0
+    ach = cheb_bytes(CHEB_ORDER, CHEB_NVEC) / t_cheb / 1e6
+    roofline = {"bound": "hbm", "kernel": "dwf::hop_tile_kernel<float,16,32,...> (H_DW and H_DW+axpby epilogues, inside dwf_chebyshev)",
                 "achieved": round(ach, 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(ach / peak, 4),
-                "traffic": None, "avg_launch_ms": round(t_cheb / n_launch, 4), "launches_per_step": n_launch,
+                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "traffic_source": NCU_TRAFFIC_SOURCE,
+                "algorithmic_bytes_per_launch": round(cheb_bytes(CHEB_ORDER, CHEB_NVEC) / n_launch),
+                "avg_launch_ms": round(t_cheb / n_launch, 4), "launches_per_call": n_launch,
+                "co_limit": "packed-fp32 FMA pipe: ~906 FFMA2/FADD2/FMUL2 per 2 5D sites, measured 100 lane-FMA/clk/SM (DESIGN.md sec. 5.2)",
                 "ddw_nrhs1_frac": detail["ddw_nrhs1"]["frac_of_hbm_peak"]}
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(prof):
-        try:
-            roofline["traffic"] = json.load(open(prof)).get("hop_kernel_cheb_bytes_per_launch")
-        except Exception:
-            pass
 
     total_flop = FLOP_PER_SITE * V5 * hop_applies["n"] * args.steps * world
     value = total_flop / ms / 1e6

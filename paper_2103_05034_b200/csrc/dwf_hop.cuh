@@ -190,11 +190,18 @@ __device__ __forceinline__ void self_term(CV<double> (&res)[12], const double2* 
     const int snext = (k == K - 1) ? 0 : k + 1;
     const double coef_dn = (k == 0) ? mass : -1.0;
     const double coef_up = (k == K - 1) ? mass : -1.0;
+    // When K divides 32 the K threads of a block sit in one warp: fetch the s-1 / s+1 lane by shuffle.
+    const bool shfl = (K == 4 || K == 8 || K == 16 || K == 32);
+    const int lane = threadIdx.x & 31;
+    const unsigned mask = __activemask();
+    const int src_dn = lane - k + sprev, src_up = lane - k + snext;
 #pragma unroll
     for (int c = 0; c < 12; c++) {
         const CV<double> own = unpack(ldg_nc(blk + c * K + k));
         const bool down = DAG ? (c >= 6) : (c < 6);
-        const CV<double> o = unpack(ldg_nc(blk + c * K + (down ? sprev : snext)));
+        CV<double> o;
+        if (shfl) { o.re = __shfl_sync(mask, own.re, down ? src_dn : src_up); o.im = __shfl_sync(mask, own.im, down ? src_dn : src_up); }
+        else o = unpack(ldg_nc(blk + c * K + (down ? sprev : snext)));
         const double coef = down ? coef_dn : coef_up;
         res[c].re = fma(coef, o.re, fma(c_diag, own.re, res[c].re));
         res[c].im = fma(coef, o.im, fma(c_diag, own.im, res[c].im));
