@@ -282,7 +282,9 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     const int K = h->Ls / Prec<R>::VL;
     // tiled persistent stencil (dwf_tile.cuh): lattice made of whole tiles, compile-time Ls, a hop to do
     const bool ls_ct = (h->Ls == 16 || h->Ls == 24);
-    const int TS = (ls_ct && k.mode != HM_SELF && h->glinks) ? h->tile_sites : 0;
+    // (its item index is 32-bit: fall back to the generic kernel for absurdly large launches)
+    const bool fits32 = h->tile_sites && 2 * (h->V4h / h->tile_sites + h->blk_sites) * (long long)h->rhs_chunk < (1LL << 31);
+    const int TS = (ls_ct && k.mode != HM_SELF && h->glinks && fits32) ? h->tile_sites : 0;
     a.sg_shift = h->sg_shift;
     a.GS = TS ? TS : std::min(HOP_THREADS / 8, HOP_THREADS / K);                                   // sites per CTA
     a.ngroups = (h->V4h + a.GS - 1) / a.GS;
