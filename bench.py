@@ -165,6 +165,29 @@ def run_only(args, dev):
     name = args.only
     if name.endswith("_48"):
         return run_only_config4(args, dev)
+    if name == "subspace":                                   # eq. 34-37 on 16^3x32x16 fp32, one noise vector
+        m, lam_lo, lam_max, delta, nvec = 64, 0.5, 60.0, 16, 5
+        d = Dwf(L, LS, M5, MASS, DWF_F32, device=dev)
+        d.set_gauge(torch.from_numpy(gen.gauge_random(L, 1002)).to(d.cdtype).to(dev))
+        d.set_workspace(1)
+        g = torch.Generator(device=dev); g.manual_seed(2007)
+        eta = d.field(1).normal_(generator=g)
+        phi = torch.empty(nvec * eta.numel(), dtype=d.rdtype, device=dev)
+        lam, _ = d.power_lambda_max(20, eta.clone())
+        for _ in range(3):
+            d.chebyshev_subspace(m, lam_lo, lam_max, delta, nvec, eta, phi, 1)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(args.steps):
+            d.chebyshev_subspace(m, lam_lo, lam_max, delta, nvec, eta, phi, 1)
+        b.record(); torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / args.steps
+        applies = 2 * m + 2 * (nvec - 1) * delta
+        print(json.dumps({"only": name, "m": m, "delta": delta, "nvec": nvec, "lambda_max_power20": round(lam, 3), "ms": round(ms, 3),
+                          "H_applies": applies, "us_per_apply": round(1e3 * ms / applies, 1), "vectors/s": round(nvec / ms * 1e3, 1),
+                          "GFlop/s": round(FLOP_PER_SITE * V5 * applies / ms / 1e6, 1)}), flush=True)
+        return
     if name == "cg_8":                                       # BASELINE.json configs[1]: 8^4 x 16, 50 rb-CG iterations (launch-bound size)
         L8 = (8, 8, 8, 8)
         d = Dwf(L8, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)

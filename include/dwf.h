@@ -66,7 +66,7 @@ int dwf_destroy(dwf_handle h);
 /* Stream on which all later work of this handle is enqueued (a cudaStream_t; NULL = default). */
 int dwf_set_stream(dwf_handle h, void* cuda_stream);
 
-/* Scratch for dwf_apply(SCHUR_EO), dwf_chebyshev, dwf_cg_schur, dwf_apply_host with up to `nrhs`
+/* Scratch for dwf_apply(SCHUR_EO), dwf_chebyshev(_subspace), dwf_power_lambda_max, dwf_cg_schur, dwf_apply_host with up to `nrhs`
  * right-hand sides.  The library never allocates field memory: the caller provides a device buffer
  * of at least dwf_workspace_bytes() bytes and keeps it alive while the handle uses it. */
 size_t dwf_workspace_bytes(dwf_handle h, int nrhs);
@@ -96,6 +96,30 @@ int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* out_host, in
 /* out = T_order(2 (H_DW^2 - lo) / (hi - lo) - 1) in   (eq. 23, eq. 34; R10, R13, R14).
  * order >= 0, hi > lo.  Full native fields; in != out; uses the workspace (2 full fields). */
 int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, const void* in, void* out, int nrhs);
+
+/* Subspace generation by Chebyshev filtering of a noise vector (eq. 34-37; setup option 3).
+ *   v     = T_m(2 (H_DW^2 - lambda_lo) / (lambda_max - lambda_lo) - 1) eta        first-pass filter, eq. 34 (R10)
+ *   phi_k = T_{k delta}(2 H_DW^2 / lambda_max - 1) v ,  k = 0 .. nvec-1            eq. 35, 37 (phi_0 = v, R23)
+ * All phi_k come from ONE three-term recurrence started at v ("all for the cost of the highest order", L229):
+ * 2 m + 2 (nvec-1) delta operator applies.  phi = nvec consecutive full native fields of nrhs right-hand sides
+ * each (phi_k at byte offset k * dwf_field_bytes(h, nrhs, 0)); eta != phi; m >= 0, delta >= 1, nvec >= 1,
+ * 0 <= lambda_lo < lambda_max.  No normalisation (R14).  Uses the workspace (3 full fields). */
+int dwf_chebyshev_subspace(dwf_handle h, int m, double lambda_lo, double lambda_max, int delta, int nvec,
+                           const void* eta, void* phi, int nrhs);
+
+/* Chebyshev smoother of degree N on the normal residual system (eq. 24-25):
+ *   out = [ c_0/2 + sum_{j=1..N} c_j T_j(2 (M^dag M - a)/(b - a) - 1) ] M^dag r ,  M = D_DW (M^dag M = H_DW^2),
+ *   c_j = (2/N) sum_{k=0..N-1} f(y(cos theta_k)) cos(j theta_k), f(y) = 1/y, theta_k = pi (k + 1/2)/N,
+ *   y(x) = ((b - a) x + b + a)/2  (the inverse of the interval map of L173): a polynomial approximation of M^-1 on
+ *   the part of the spectrum of M^dag M inside [a, b].  1 <= N <= 4096, 0 < a < b; r != out; full native fields.
+ * Uses the workspace (4 full fields). */
+int dwf_chebyshev_smoother(dwf_handle h, int N, double a, double b, const void* r, void* out, int nrhs);
+
+/* lambda_max(H_DW^2) by the power method (L225; reading R24), nrhs = 1, full native field v (start vector in,
+ * last iterate out).  Iteration i: u = H v, lambda_i = |u|^2 / |v|^2 (Rayleigh quotient of H^2),
+ * v <- H u / lambda_i.  *lambda_host = lambda_iters; lambda_hist_host (may be NULL) receives all `iters`
+ * quotients.  Uses the workspace (2 full fields).  Synchronises. */
+int dwf_power_lambda_max(dwf_handle h, int iters, void* v, double* lambda_host, double* lambda_hist_host);
 
 /* BLAS-1 on native fields (half = 0 full, 1 half field), one scalar per right-hand side.
  *   axpy : y <- a x + y, a_host[2*nrhs] = (re, im) per rhs

@@ -159,6 +159,41 @@ def chebyshev(U, psi, M5: float, mass: float, order: int, lo: float, hi: float) 
     return out
 
 
+def chebyshev_subspace(U, eta, M5: float, mass: float, m: int, lam_lo: float, lam_max: float, delta: int, nvec: int):
+    """Setup option 3 of the paper (L221-241): first-pass filter v = T_m(2(M^dag M - lam_lo)/(lam_max - lam_lo) - 1) eta
+    (eq. 34, reading R10) and phi_k = T_{k delta}(2 M^dag M/lam_max - 1) v, k = 0..nvec-1 (eq. 35, 37; phi_0 = v, R23).
+    Written as the definition: every phi_k is its own polynomial of the pinned `chebyshev` (the shared recurrence that
+    makes them "all for the cost of the highest order" is the GPU path's business).  Returns [nvec, *eta.shape]."""
+    v = chebyshev(U, eta, M5, mass, m, lam_lo, lam_max)
+    return np.stack([chebyshev(U, v, M5, mass, k * delta, 0.0, lam_max) for k in range(nvec)])
+
+
+def chebyshev_smoother(U, r, M5: float, mass: float, N: int, a: float, b: float) -> np.ndarray:
+    """S r = [c_0/2 + sum_{j=1..N} c_j T_j(2(M^dag M - a)/(b-a) - 1)] M^dag r (eq. 24), c_j by eq. 25 with f(y) = 1/y,
+    theta_k = pi (k+1/2)/N; y(x) inverts the interval map of L173.  Term by term through the pinned `chebyshev`."""
+    th = np.pi * (np.arange(N) + 0.5) / N
+    y = 0.5 * ((b - a) * np.cos(th) + (b + a))
+    c = [2.0 / N * np.sum(np.cos(j * th) / y) for j in range(N + 1)]
+    v = ddw(U, r, M5, mass, dagger=True)
+    out = 0.5 * c[0] * v
+    for j in range(1, N + 1):
+        out = out + c[j] * chebyshev(U, v, M5, mass, j, a, b)
+    return out
+
+
+def power_lambda_max(U, v0, M5: float, mass: float, iters: int):
+    """Power method for lambda_max(M^dag M) (L225; reading R24): u = H v, lambda_i = |u|^2/|v|^2, v <- H u / lambda_i.
+    Returns (list of the `iters` Rayleigh quotients, last iterate)."""
+    v = _c(v0)
+    hist = []
+    for _ in range(iters):
+        u = hdw(U, v, M5, mass)
+        lam = float(np.vdot(u, u).real / np.vdot(v, v).real)
+        hist.append(lam)
+        v = hdw(U, u, M5, mass) / lam
+    return hist, v
+
+
 def cg_schur(U, b_e, M5: float, mass: float, iters: int, x0=None):
     """`iters` iterations of CG on M_pc^dag M_pc x = b (eq. 9). Returns (x, |r_k|^2 history)."""
     b = _c(b_e); U = _c(U); L, Ls, nrhs = _geom(b)

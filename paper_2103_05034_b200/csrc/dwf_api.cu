@@ -181,7 +181,7 @@ extern "C" size_t dwf_field_bytes(dwf_handle h, int nrhs, int half) {
 }
 extern "C" size_t dwf_workspace_bytes(dwf_handle h, int nrhs) {
     if (!h || nrhs < 1) return 0;
-    return 5 * half_bytes(h, nrhs) + 256;
+    return 8 * half_bytes(h, nrhs) + 256;          // dwf_chebyshev_smoother: 4 full fields
 }
 extern "C" int dwf_set_workspace(dwf_handle h, void* p, size_t n) {
     if (!h) return DWF_EINVAL;
@@ -472,6 +472,128 @@ extern "C" int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, cons
         if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, 2.0 * alpha, tk, -2.0 * beta, tkm1, -1.0)) return rc;
         tkm1 = tk; tk = dst;
     }
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Subspace generation by Chebyshev filtering (eq. 34-37).
+//   first pass : v = T_m(2(H^2 - lambda_lo)/(lambda_max - lambda_lo) - 1) eta                 (eq. 34, reading R10)
+//   then ONE recurrence in X' = 2 H^2/lambda_max - 1 started from v, emitting
+//   phi_k = T_{k Delta}(X') v  for k = 0 .. nvec-1  ("all for the cost of the highest order", L229; eq. 37)
+// phi: nvec consecutive full native fields of nrhs right-hand sides each.  Workspace: 3 full fields.
+// ------------------------------------------------------------------------------------------------
+extern "C" int dwf_chebyshev_subspace(dwf_handle h, int m, double lambda_lo, double lambda_max, int delta, int nvec,
+                                      const void* eta, void* phi, int nrhs) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
+    if (m < 0 || delta < 1 || nvec < 1 || !(lambda_max > lambda_lo) || !(lambda_lo >= 0.0)) FAIL(h, DWF_EINVAL, "need m >= 0, delta >= 1, nvec >= 1, 0 <= lambda_lo < lambda_max");
+    if (int rc = check_field(h, eta, "eta")) return rc;
+    if (int rc = check_field(h, phi, "phi")) return rc;
+    if (eta == phi) FAIL(h, DWF_EINVAL, "eta == phi");
+    if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    const size_t fb = 2 * half_bytes(h, nrhs);
+    if (int rc = need_ws(h, 3 * fb)) return rc;
+    // first pass straight into phi_0 (dwf_chebyshev uses workspace fields 0 and 1)
+    if (int rc = dwf_chebyshev(h, m, lambda_lo, lambda_max, eta, phi, nrhs)) return rc;
+    if (nvec == 1) return DWF_OK;
+    void* w = h->ws; void* A = (char*)h->ws + fb; void* B = (char*)h->ws + 2 * fb;
+    const double alpha = 2.0 / lambda_max, beta = 1.0;                          // X' = alpha H^2 - beta
+    const void* t0 = phi;
+    if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, t0, w, nrhs)) return rc;
+    if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, A, nrhs, alpha, t0, -beta, t0, 0.0)) return rc;
+    const void* tkm1 = t0; void* tk = A;
+    const int last = (nvec - 1) * delta;
+    for (int k = 1; ; k++) {                                                   // tk = t_k
+        if (k % delta == 0)
+            CUDA_TRY(h, cudaMemcpyAsync((char*)phi + (size_t)(k / delta) * fb, tk, fb, cudaMemcpyDeviceToDevice, h->stream));
+        if (k == last) break;
+        void* dst = (k == 1) ? B : (void*)tkm1;                                 // t_{k+1} overwrites t_{k-1} (t_0 = phi_0 is kept)
+        if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, tk, w, nrhs)) return rc;
+        if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, 2.0 * alpha, tk, -2.0 * beta, tkm1, -1.0)) return rc;
+        tkm1 = tk; tk = dst;
+    }
+    return DWF_OK;
+}
+
+// Chebyshev smoother (eq. 24-25):
+//   out = [ c_0/2 + sum_{j=1..N} c_j T_j(2(M^dag M - a)/(b - a) - 1) ] M^dag r ,   M = D_DW,  M^dag M = H_DW^2,
+//   c_j = (2/N) sum_{k<N} f(y(cos theta_k)) cos(j theta_k),  f(y) = 1/y,  theta_k = pi (k + 1/2)/N,
+//   y(x) = ((b - a) x + (b + a))/2.
+// v = M^dag r by the adjoint stencil, then the three-term recurrence of dwf_chebyshev with a forward summation
+// (one axpy per order).  Workspace: 4 full fields (v, w, t_odd, t_even).
+extern "C" int dwf_chebyshev_smoother(dwf_handle h, int N, double a, double b, const void* r, void* out, int nrhs) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
+    if (N < 1 || N > 4096 || !(b > a) || !(a > 0.0)) FAIL(h, DWF_EINVAL, "need 1 <= N <= 4096 and 0 < a < b");
+    if (int rc = check_field(h, r, "r")) return rc;
+    if (int rc = check_field(h, out, "out")) return rc;
+    if (r == out) FAIL(h, DWF_EINVAL, "r == out");
+    if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    const size_t fb = 2 * half_bytes(h, nrhs);
+    if (int rc = need_ws(h, 4 * fb)) return rc;
+    std::vector<double> c(N + 1);
+    const double pi = 3.14159265358979323846;
+    for (int j = 0; j <= N; j++) {
+        double acc = 0;
+        for (int k = 0; k < N; k++) {
+            const double th = pi * (k + 0.5) / N;
+            const double y = 0.5 * ((b - a) * std::cos(th) + (b + a));
+            acc += std::cos(j * th) / y;
+        }
+        c[j] = 2.0 * acc / N;
+    }
+    void* v = h->ws; void* w = (char*)h->ws + fb; void* A = (char*)h->ws + 2 * fb; void* B = (char*)h->ws + 3 * fb;
+    double coef[2 * MAX_NRHS];
+    auto add = [&](double cj, const void* t) -> int {                          // out += cj t
+        for (int q = 0; q < nrhs; q++) { coef[2 * q] = cj; coef[2 * q + 1] = 0.0; }
+        return dwf_axpy(h, coef, t, out, nrhs, 0);
+    };
+    if (int rc = full_op(h, HM_HOP_SELF, true, -0.5, h->mass, r, v, nrhs)) return rc;           // v = D_DW^dag r
+    CUDA_TRY(h, cudaMemsetAsync(out, 0, fb, h->stream));
+    if (int rc = add(0.5 * c[0], v)) return rc;
+    const double alpha = 2.0 / (b - a), beta = (b + a) / (b - a);
+    if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, v, w, nrhs)) return rc;
+    if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, A, nrhs, alpha, v, -beta, v, 0.0)) return rc;
+    if (int rc = add(c[1], A)) return rc;
+    const void* tkm1 = v; void* tk = A;
+    for (int k = 1; k < N; k++) {
+        void* dst = (k == 1) ? B : (void*)tkm1;
+        if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, tk, w, nrhs)) return rc;
+        if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, 2.0 * alpha, tk, -2.0 * beta, tkm1, -1.0)) return rc;
+        tkm1 = tk; tk = dst;
+        if (int rc = add(c[k + 1], tk)) return rc;
+    }
+    return DWF_OK;
+}
+
+// lambda_max(H_DW^2) by the power method (L225), nrhs = 1.  v holds the start vector on entry and the last
+// iterate on return.  Iteration i: u = H v; lambda_i = |u|^2/|v|^2 (Rayleigh quotient of H^2); v <- H u / lambda_i
+// (keeps |v| = O(1)).  lambda_hist_host (may be NULL) receives the `iters` quotients; returns the last in *lambda_host.
+// Workspace: 2 full fields.
+extern "C" int dwf_power_lambda_max(dwf_handle h, int iters, void* v, double* lambda_host, double* lambda_hist_host) {
+    if (!h) return DWF_EINVAL;
+    if (iters < 1 || !lambda_host) FAIL(h, DWF_EINVAL, "need iters >= 1 and lambda_host");
+    if (int rc = check_field(h, v, "v")) return rc;
+    if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    const size_t fb = 2 * half_bytes(h, 1);
+    if (int rc = need_ws(h, 2 * fb)) return rc;
+    void* u = h->ws; void* vn = (char*)h->ws + fb;
+    void* cur = v; void* nxt = vn;
+    double lam = 0.0;
+    for (int i = 0; i < iters; i++) {
+        if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, cur, u, 1)) return rc;
+        double nu = 0, nv = 0;
+        if (int rc = dwf_norm2(h, u, &nu, 1, 0)) return rc;
+        if (int rc = dwf_norm2(h, cur, &nv, 1, 0)) return rc;
+        if (!(nv > 0.0) || !(nu > 0.0)) FAIL(h, DWF_EINVAL, "power method: zero vector");
+        lam = nu / nv;
+        if (lambda_hist_host) lambda_hist_host[i] = lam;
+        if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, u, nxt, 1, 1.0 / lam, u, 0.0, u, 0.0)) return rc;
+        std::swap(cur, nxt);
+    }
+    if (cur != v) CUDA_TRY(h, cudaMemcpyAsync(v, cur, fb, cudaMemcpyDeviceToDevice, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    *lambda_host = lam;
     return DWF_OK;
 }
 

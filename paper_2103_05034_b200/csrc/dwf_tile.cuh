@@ -218,6 +218,7 @@ hop_tile_kernel(const HopArgs<R> a) {
             auto release_buffers = [&]() {
                 __syncwarp();
                 if ((threadIdx.x & 31) == 0) {
+                    __threadfence_block();                     // this warp's reads of the buffers are performed before it counts itself done
                     const unsigned prev = atomicAdd(done_count + buf, 1u);
                     if (prev == (unsigned)((it >> 1) + 1) * NWARPS - 1) {
                         if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);

@@ -35,6 +35,12 @@ _SIGNATURES = {
     "dwf_apply_host": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
     "dwf_chebyshev": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double,
                                      ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dwf_chebyshev_subspace": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+                                              ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dwf_chebyshev_smoother": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_double,
+                                              ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dwf_power_lambda_max": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double),
+                                            ctypes.POINTER(ctypes.c_double)]),
     "dwf_axpy": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_void_p, ctypes.c_void_p,
                                 ctypes.c_int, ctypes.c_int]),
     "dwf_inner": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double),
@@ -179,6 +185,24 @@ class Dwf:
     def chebyshev(self, order: int, lo: float, hi: float, inp: torch.Tensor, out: torch.Tensor, nrhs: int) -> torch.Tensor:
         self._check(self.lib.dwf_chebyshev(self._h, order, lo, hi, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr()), nrhs))
         return out
+
+    def chebyshev_subspace(self, m: int, lambda_lo: float, lambda_max: float, delta: int, nvec: int, eta: torch.Tensor,
+                           phi: torch.Tensor, nrhs: int) -> torch.Tensor:
+        """phi: 1-D native tensor of nvec * field elements (phi_k = phi[k * n : (k + 1) * n])."""
+        assert phi.numel() == nvec * eta.numel()
+        self._check(self.lib.dwf_chebyshev_subspace(self._h, m, lambda_lo, lambda_max, delta, nvec, ctypes.c_void_p(eta.data_ptr()),
+                                                    ctypes.c_void_p(phi.data_ptr()), nrhs))
+        return phi
+
+    def chebyshev_smoother(self, N: int, a: float, b: float, r: torch.Tensor, out: torch.Tensor, nrhs: int) -> torch.Tensor:
+        self._check(self.lib.dwf_chebyshev_smoother(self._h, N, a, b, ctypes.c_void_p(r.data_ptr()), ctypes.c_void_p(out.data_ptr()), nrhs))
+        return out
+
+    def power_lambda_max(self, iters: int, v: torch.Tensor):
+        lam = ctypes.c_double()
+        hist = (ctypes.c_double * iters)()
+        self._check(self.lib.dwf_power_lambda_max(self._h, iters, ctypes.c_void_p(v.data_ptr()), ctypes.byref(lam), hist))
+        return float(lam.value), [float(x) for x in hist]
 
     def axpy(self, a, x: torch.Tensor, y: torch.Tensor, nrhs: int, half: bool = False):
         a = [complex(v) for v in a]

@@ -152,3 +152,59 @@ def test_abi_errors():
     d2 = Dwf((4, 4, 4, 4), 10, M5, 0.01, DWF_F64)
     with pytest.raises(DwfError, match="instantiated"):
         d2.apply(DWF_MOOINV, d2.field(1, half=True), d2.field(1, half=True), 1)   # Ls = 10 unsupported
+
+
+# ------------------------------------------------------------------ subspace generation + power method
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_chebyshev_subspace(oracle, prec):
+    L, Ls, mass, nrhs = (4, 4, 4, 8), 8, 0.01, 2
+    m, lam_lo, lam_max, delta, nvec = 12, 0.5, 60.0, 5, 4           # lam_lo inside the spectrum: the first pass amplifies
+    rig = Rig(L, Ls, prec, mass, seed_U=1000, ws_nrhs=nrhs)
+    eta = rig.spinor(nrhs, 2005)
+    xn = rig.native(eta)
+    phi = torch_empty_like_fields(rig, nvec, nrhs)
+    rig.d.chebyshev_subspace(m, lam_lo, lam_max, delta, nvec, xn, phi, nrhs)
+    want = oracle.chebyshev_subspace(rig.U, eta, M5, mass, m, lam_lo, lam_max, delta, nvec)
+    n = xn.numel()
+    for k in range(nvec):
+        got = rig.canonical(phi[k * n:(k + 1) * n], nrhs)
+        assert rel_l2(got, want[k]) < (1e-11 if prec == "f64" else 1e-4), k
+    assert np.array_equal(rig.canonical(xn, nrhs), eta)               # input untouched
+    # nvec = 1 is the first-pass filter alone
+    one = torch_empty_like_fields(rig, 1, nrhs)
+    rig.d.chebyshev_subspace(m, lam_lo, lam_max, delta, 1, xn, one, nrhs)
+    assert rel_l2(rig.canonical(one, nrhs), want[0]) < (1e-11 if prec == "f64" else 1e-4)
+
+
+def torch_empty_like_fields(rig, nvec, nrhs):
+    import torch
+    return torch.empty(nvec * rig.d.field(nrhs).numel(), dtype=rig.d.rdtype, device="cuda")
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_power_lambda_max(oracle, prec):
+    L, Ls, mass = (4, 4, 4, 8), 8, 0.01
+    rig = Rig(L, Ls, prec, mass, seed_U=1000, ws_nrhs=1)
+    v0 = rig.spinor(1, 2006)
+    vn = rig.native(v0)
+    lam, hist = rig.d.power_lambda_max(30, vn)
+    h_or, v_or = oracle.power_lambda_max(rig.U, v0, M5, mass, 30)
+    tol = 1e-11 if prec == "f64" else 2e-5
+    assert np.max(np.abs(np.array(hist) - np.array(h_or)) / np.array(h_or)) < tol
+    assert lam == hist[-1] and 40 < lam < 70                          # random links: lambda_max ~ 48
+    assert rel_l2(rig.canonical(vn, 1), v_or) < (1e-9 if prec == "f64" else 1e-3)
+
+
+# ------------------------------------------------------------------ Chebyshev smoother (eq. 24-25)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_chebyshev_smoother(oracle, prec):
+    L, Ls, mass, nrhs = (4, 4, 4, 8), 8, 0.01, 2
+    N, a, b = 12, 0.5, 60.0                                           # Table I of the paper: Chebyshev [0.5, 60], order 12
+    rig = Rig(L, Ls, prec, mass, seed_U=1000, ws_nrhs=nrhs)
+    r = rig.spinor(nrhs, 2008)
+    rn = rig.native(r)
+    out = rig.d.field(nrhs)
+    rig.d.chebyshev_smoother(N, a, b, rn, out, nrhs)
+    want = oracle.chebyshev_smoother(rig.U, r, M5, mass, N, a, b)
+    assert rel_l2(rig.canonical(out, nrhs), want) < (1e-11 if prec == "f64" else 1e-4)
+    assert np.array_equal(rig.canonical(rn, nrhs), r)

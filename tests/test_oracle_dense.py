@@ -140,6 +140,70 @@ def test_chebyshev_composition_identity(oracle):
     assert 0.6 < ratio < 0.8
 
 
+# ---------------------------------------------------------------- subspace generation (eq. 34-37) and power method (L225)
+def test_subspace_vs_eigendecomposition(oracle):
+    """phi_k = V T_{k Delta}(2 lam/lam_max - 1) T_m(2 (lam - lam_lo)/(lam_max - lam_lo) - 1) V^dag eta  (eq. 37, R10), with
+    lam_lo ABOVE the lowest eigenvalues so that the first pass really amplifies them (cosh branch of eq. 23)."""
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    eta = gen.spinor_gaussian(L, Ls, 1, 7)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    lam, V = np.linalg.eigh(D.conj().T @ D)
+    lam_max, m, delta, nvec = 1.05 * lam[-1], 9, 3, 4
+    lam_lo = lam[len(lam) // 8]                       # 1/8 of the spectrum lies below the low-pass value
+    cheb = lambda n, x: np.where(np.abs(x) <= 1, np.cos(n * np.arccos(np.clip(x, -1, 1))),
+                                 np.sign(x) ** n * np.cosh(n * np.arccosh(np.maximum(np.abs(x), 1))))
+    x1 = 2 * (lam - lam_lo) / (lam_max - lam_lo) - 1
+    x2 = 2 * lam / lam_max - 1
+    assert x1.min() < -1 and np.all(np.abs(x2) <= 1)
+    got = oracle.chebyshev_subspace(U, eta, M5, MASS, m, lam_lo, lam_max, delta, nvec)
+    c = V.conj().T @ eta[0].reshape(-1)
+    for k in range(nvec):
+        want = V @ (cheb(k * delta, x2) * cheb(m, x1) * c)
+        assert rel(got[k, 0].reshape(-1), want) < 1e-11
+    # the first pass enhances the low modes relative to the band (the point of the filter, L225)
+    low = np.abs(V[:, :4].conj().T @ got[0, 0].reshape(-1)) / np.abs(c[:4])
+    assert np.all(low > 1.0) and np.all(np.abs(cheb(m, x1[len(lam) // 2:])) <= 1 + 1e-12)
+
+
+def test_chebyshev_smoother_vs_library_interpolant(oracle):
+    """eq. 24-25: c_N vanishes identically (cos(N theta_k) = 0), so the smoother polynomial is THE degree N-1 Chebyshev
+    interpolant of 1/y at the N first-kind nodes of [a, b] -- numpy's chebinterpolate, evaluated on the dense spectrum.
+    And it is what a smoother should be: S M x ~ x with error max |1 - lam p(lam)| over the spectrum."""
+    from numpy.polynomial import chebyshev as npcheb
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    r = gen.spinor_gaussian(L, Ls, 2, 9)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    lam, V = np.linalg.eigh(D.conj().T @ D)
+    a, b, N = 0.9 * lam[0], 1.1 * lam[-1], 24
+    coef = npcheb.chebinterpolate(lambda x: 2.0 / ((b - a) * x + (b + a)), N - 1)
+    p = npcheb.chebval(2 * (lam - a) / (b - a) - 1, coef)
+    got = oracle.chebyshev_smoother(U, r, M5, MASS, N, a, b)
+    for q in range(2):
+        want = V @ (p * (V.conj().T @ (D.conj().T @ r[q].reshape(-1))))
+        assert rel(got[q].reshape(-1), want) < 1e-11
+    x = gen.spinor_gaussian(L, Ls, 1, 10)
+    sm = oracle.chebyshev_smoother(U, oracle.ddw(U, x, M5, MASS), M5, MASS, N, a, b)
+    eps = np.max(np.abs(1 - lam * p))
+    assert rel(sm, x) <= eps * (1 + 1e-9) and eps < 0.9
+
+
+def test_power_method_converges_to_dense_lambda_max(oracle):
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    v0 = gen.spinor_gaussian(L, Ls, 1, 8)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    lam = np.linalg.eigvalsh(D.conj().T @ D)
+    hist, v = oracle.power_lambda_max(U, v0, M5, MASS, 200)
+    assert np.all(np.diff(hist) > -1e-12 * lam[-1])                 # Rayleigh quotients of a power iteration never decrease
+    assert hist[-1] <= lam[-1] * (1 + 1e-12) and hist[-1] > 0.999 * lam[-1]
+    # first quotient is the plain Rayleigh quotient of the start vector
+    x = v0[0].reshape(-1)
+    assert abs(hist[0] - (np.vdot(D @ x, D @ x) / np.vdot(x, x)).real) / hist[0] < 1e-12
+    assert 0.1 < np.linalg.norm(v) / np.linalg.norm(v0) < 10        # the iterate stays O(1)
+
+
 # ---------------------------------------------------------------- CG (eq. 9)
 def test_cg_against_dense_solve_and_properties(oracle):
     L, Ls = (4, 2, 2, 2), 4
