@@ -134,6 +134,14 @@ int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs, int half)
  * iters+1 values |r_k|^2.  Uses the workspace (5 half fields).  Synchronises at the end only. */
 int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, double* resid2_hist_host);
 
+/* Complete red-black solve of D_DW psi = eta (Table V; eq. 9), nrhs = 1, full native fields:
+ *   eta'_e = eta_e - M_eo M_oo^-1 eta_o;  CGNR on M_pc^dag M_pc psi_e = M_pc^dag eta'_e from psi_e = 0, stopped when
+ *   |r_k| <= tol |r_0| (r = residual of the normal equations; tested every 10 iterations) or after max_iters;
+ *   psi_o = M_oo^-1 (eta_o - M_oe psi_e).
+ * *iters_host = CG iterations done; *relres_host (may be NULL) = |D_DW psi - eta| / |eta| recomputed with the
+ * full-lattice operator.  eta != psi.  Uses the workspace (8 half fields).  Synchronises. */
+int dwf_solve(dwf_handle h, const void* eta, void* psi, double tol, int max_iters, int* iters_host, double* relres_host);
+
 /* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
 long long dwf_launch_count(dwf_handle h);
 

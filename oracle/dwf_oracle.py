@@ -181,6 +181,35 @@ def chebyshev_smoother(U, r, M5: float, mass: float, N: int, a: float, b: float)
     return out
 
 
+def _parity_mask(L, parity: int) -> np.ndarray:
+    Lx, Ly, Lz, Lt = L
+    t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
+    return (((x + y + z + t) & 1) == parity)[None, None, :, :, :, :, None, None]
+
+
+def solve_rb(U, eta, M5: float, mass: float, tol: float, max_iters: int, check_every: int = 10):
+    """D_DW psi = eta by the complete red-black solve (Table V, eq. 9), nrhs = 1:
+    eta'_e = eta_e - M_eo M_oo^-1 eta_o; CGNR on M_pc^dag M_pc psi_e = M_pc^dag eta'_e from 0, stopped at the first
+    multiple of `check_every` iterations with |r_k| <= tol |r_0| (or max_iters); psi_o = M_oo^-1 (eta_o - M_oe psi_e);
+    M_eo = M_oe = -1/2 Dhop (eq. 4-5).  Returns (psi, iterations)."""
+    eta = _c(eta); L, Ls, _ = _geom(eta)
+    me, mo = _parity_mask(L, 0), _parity_mask(L, 1)
+    eta_e, eta_o = eta * me, eta * mo
+    m_eo = lambda f_o: -0.5 * dhop(U, f_o, row_parity=0)            # onto even sites
+    m_oe = lambda f_e: -0.5 * dhop(U, f_e, row_parity=1)            # onto odd sites
+    src = eta_e - m_eo(mpp_inv(eta_o, M5, mass, 1))
+    b = mpc(U, src, M5, mass, dagger=True)
+    _, hist = cg_schur(U, b, M5, mass, max_iters)
+    iters = max_iters
+    for k in range(check_every, max_iters + 1, check_every):
+        if hist[k] <= tol * tol * hist[0]:
+            iters = k
+            break
+    psi_e, _ = cg_schur(U, b, M5, mass, iters)
+    psi_o = mpp_inv(eta_o - m_oe(psi_e), M5, mass, 1)
+    return psi_e * me + psi_o * mo, iters
+
+
 def power_lambda_max(U, v0, M5: float, mass: float, iters: int):
     """Power method for lambda_max(M^dag M) (L225; reading R24): u = H v, lambda_i = |u|^2/|v|^2, v <- H u / lambda_i.
     Returns (list of the `iters` Rayleigh quotients, last iterate)."""

@@ -671,7 +671,7 @@ extern "C" int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs
 // <p_k, A p_k> = |M p_k|^2 at scal[iters+1+k].
 // ------------------------------------------------------------------------------------------------
 template <typename R>
-static int cg_t(dwf_ctx* h, const void* b, void* x, int iters) {
+static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, double tol_rel = 0.0, int check_every = 10, int* done = nullptr) {
     using G = typename Prec<R>::G;
     const size_t hb = half_bytes(h, 1);
     const long long ng = half_groups(h, 1);
@@ -691,6 +691,13 @@ static int cg_t(dwf_ctx* h, const void* b, void* x, int iters) {
         cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, hist + k, pAp + k, h->partial); LAUNCH_CHECK(h);
         reduce_final_kernel<<<1, 64, 0, st>>>(h->partial, (int)blocks, 1, hist + k + 1, 1, 1); LAUNCH_CHECK(h);
         cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, hist + k + 1, hist + k); LAUNCH_CHECK(h);
+        if (done) *done = k + 1;
+        if (tol_rel > 0.0 && ((k + 1) % check_every == 0 || k + 1 == iters)) {      // stopping test: |r_k|^2 <= tol^2 |r_0|^2
+            CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, hist, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(h, cudaMemcpyAsync(h->scal_host + 1, hist + k + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(h, cudaStreamSynchronize(st));
+            if (h->scal_host[1] <= tol_rel * tol_rel * h->scal_host[0]) break;
+        }
     }
     return DWF_OK;
 }
@@ -732,6 +739,62 @@ extern "C" int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int 
     CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, (iters + 1) * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (hist_host) memcpy(hist_host, h->scal_host, (iters + 1) * sizeof(double));
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Complete red-black solve of D_DW psi = eta (Table V, eq. 9), nrhs = 1:
+//   eta'_e = eta_e - M_eo M_oo^-1 eta_o ;  CGNR: M_pc^dag M_pc psi_e = M_pc^dag eta'_e (stop: |r_k| <= tol |r_0|, tested
+//   every 10 iterations) ;  psi_o = M_oo^-1 (eta_o - M_oe psi_e) ;  M_eo = M_oe = -1/2 Dhop.
+// Workspace halves: [0,5) CG, 5: b, 6: t / Schur scratch, 7: hop scratch.  psi_o doubles as scratch until the end.
+// ------------------------------------------------------------------------------------------------
+extern "C" int dwf_solve(dwf_handle h, const void* eta, void* psi, double tol, int max_iters, int* iters_host, double* relres_host) {
+    if (!h) return DWF_EINVAL;
+    if (!(tol > 0.0) || max_iters < 1 || 2 * max_iters + 2 > SCAL_DOUBLES) FAIL(h, DWF_EINVAL, "need tol > 0 and 1 <= max_iters <= %d", SCAL_DOUBLES / 2 - 1);
+    if (int rc = check_field(h, eta, "eta")) return rc;
+    if (int rc = check_field(h, psi, "psi")) return rc;
+    if (eta == psi) FAIL(h, DWF_EINVAL, "eta == psi");
+    if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    const size_t hb = half_bytes(h, 1);
+    if (int rc = need_ws(h, 8 * hb)) return rc;
+    const char* eta_e = (const char*)eta; const char* eta_o = eta_e + hb;
+    char* psi_e = (char*)psi; char* psi_o = psi_e + hb;
+    char* B = (char*)h->ws + 5 * hb; char* T = (char*)h->ws + 6 * hb; char* W = (char*)h->ws + 7 * hb;
+    const double half[2] = {0.5, 0.0};
+    auto hop_to = [&](int parity_out, const void* in, void* out) -> int {       // out_p = Dhop in_{1-p}
+        HopCall k{}; k.mode = HM_HOP; k.dag = false; k.nslots = 1; k.parity0 = parity_out; k.nrhs = 1;
+        k.in_hop[0] = in; k.out[0] = out; k.c_hop = 1.0; k.mass = h->mass;
+        return launch_hop(h, k);
+    };
+    // source preparation
+    if (int rc = launch_mooinv(h, eta_o, T, 1, h->mass, false)) return rc;
+    if (int rc = hop_to(0, T, W)) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(psi_o, eta_e, hb, cudaMemcpyDeviceToDevice, h->stream));
+    if (int rc = dwf_axpy(h, half, W, psi_o, 1, 1)) return rc;                   // eta'_e = eta_e + 1/2 Dhop_eo M_oo^-1 eta_o
+    if (int rc = schur_op(h, true, psi_o, B, T, 1)) return rc;                   // b = M_pc^dag eta'_e
+    // CGNR from x_0 = 0
+    CUDA_TRY(h, cudaMemsetAsync(psi_e, 0, hb, h->stream));
+    int done = 0;
+    int rc = h->prec == DWF_F32 ? cg_t<float>(h, B, psi_e, max_iters, tol, 10, &done) : cg_t<double>(h, B, psi_e, max_iters, tol, 10, &done);
+    if (rc) return rc;
+    // reconstruction of the odd sites
+    if (int rc2 = hop_to(1, psi_e, W)) return rc2;
+    CUDA_TRY(h, cudaMemcpyAsync(T, eta_o, hb, cudaMemcpyDeviceToDevice, h->stream));
+    if (int rc2 = dwf_axpy(h, half, W, T, 1, 1)) return rc2;                     // eta_o + 1/2 Dhop_oe psi_e
+    if (int rc2 = launch_mooinv(h, T, psi_o, 1, h->mass, false)) return rc2;
+    // true residual |D_DW psi - eta| / |eta| with the full-lattice operator
+    if (relres_host) {
+        void* Rf = h->ws;
+        if (int rc2 = full_op(h, HM_HOP_SELF, false, -0.5, h->mass, psi, Rf, 1)) return rc2;
+        const double minus[2] = {-1.0, 0.0};
+        if (int rc2 = dwf_axpy(h, minus, eta, Rf, 1, 0)) return rc2;
+        double nr = 0, ne = 0;
+        if (int rc2 = dwf_norm2(h, Rf, &nr, 1, 0)) return rc2;
+        if (int rc2 = dwf_norm2(h, eta, &ne, 1, 0)) return rc2;
+        *relres_host = std::sqrt(nr / ne);
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (iters_host) *iters_host = done;
     return DWF_OK;
 }
 

@@ -49,6 +49,8 @@ _SIGNATURES = {
                                  ctypes.c_int]),
     "dwf_cg_schur": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
                                     ctypes.POINTER(ctypes.c_double)]),
+    "dwf_solve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_int,
+                                 ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]),
     "dwf_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "dwf_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
 }
@@ -227,6 +229,13 @@ class Dwf:
         hist = (ctypes.c_double * (iters + 1))()
         self._check(self.lib.dwf_cg_schur(self._h, ctypes.c_void_p(b_even.data_ptr()), ctypes.c_void_p(x_even.data_ptr()), iters, hist))
         return [float(v) for v in hist]
+
+    def solve(self, eta: torch.Tensor, psi: torch.Tensor, tol: float, max_iters: int):
+        """D_DW psi = eta by the complete red-black CGNR solve; returns (iterations, true relative residual)."""
+        it, rr = ctypes.c_int(), ctypes.c_double()
+        self._check(self.lib.dwf_solve(self._h, ctypes.c_void_p(eta.data_ptr()), ctypes.c_void_p(psi.data_ptr()), tol, max_iters,
+                                       ctypes.byref(it), ctypes.byref(rr)))
+        return int(it.value), float(rr.value)
 
     def launch_count(self) -> int:
         return int(self.lib.dwf_launch_count(self._h))

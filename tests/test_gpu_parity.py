@@ -208,3 +208,21 @@ def test_chebyshev_smoother(oracle, prec):
     want = oracle.chebyshev_smoother(rig.U, r, M5, mass, N, a, b)
     assert rel_l2(rig.canonical(out, nrhs), want) < (1e-11 if prec == "f64" else 1e-4)
     assert np.array_equal(rig.canonical(rn, nrhs), r)
+
+
+# ------------------------------------------------------------------ complete red-black solve
+@pytest.mark.parametrize("prec,tol", [("f64", 1e-10), ("f32", 1e-5)])
+def test_solve_red_black(oracle, prec, tol):
+    L, Ls, mass = (4, 4, 4, 8), 8, 0.05
+    rig = Rig(L, Ls, prec, mass, seed_U=1000, ws_nrhs=1)
+    eta = rig.spinor(1, 2009)
+    en = rig.native(eta)
+    psi = rig.d.field(1)
+    iters, relres = rig.d.solve(en, psi, tol, 2000)
+    psi_or, it_or = oracle.solve_rb(rig.U, eta, M5, mass, tol, 2000)
+    got = rig.canonical(psi, 1)
+    assert iters < 2000 and abs(iters - it_or) <= 10                   # same stopping rule; the test sits every 10 iterations
+    assert relres < 30 * tol                                           # true residual of the original system
+    assert rel_l2(oracle.ddw(rig.U, got, M5, mass), eta) < 30 * tol    # ... and the oracle's operator agrees
+    assert rel_l2(got, psi_or) < 100 * tol
+    assert np.array_equal(rig.canonical(en, 1), eta)

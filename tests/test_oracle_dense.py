@@ -233,3 +233,20 @@ def test_cg_against_dense_solve_and_properties(oracle):
     x20, _ = oracle.cg_schur(U, b, M5, MASS, 20)
     x20b, h2 = oracle.cg_schur(U, b, M5, MASS, 130, x0=x20)
     assert rel(x20b[0].reshape(-1)[e], xs) < 1e-9
+
+
+# ---------------------------------------------------------------- complete red-black solve (Table V)
+def test_solve_rb_against_dense_solve(oracle):
+    """The red-black solve returns THE solution of D_DW psi = eta: dense numpy solve, and the residual through the pinned ddw."""
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    eta = gen.spinor_gaussian(L, Ls, 1, 11)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    want = np.linalg.solve(D, eta[0].reshape(-1))
+    psi, iters = oracle.solve_rb(U, eta, M5, MASS, 1e-13, 400)
+    assert iters < 400 and iters % 10 == 0
+    assert rel(psi[0].reshape(-1), want) < 1e-9
+    assert rel(oracle.ddw(U, psi, M5, MASS), eta) < 1e-10
+    loose, it2 = oracle.solve_rb(U, eta, M5, MASS, 1e-3, 400)
+    assert it2 < iters and 1e-7 < rel(oracle.ddw(U, loose, M5, MASS), eta) < 1e-1     # the tolerance is what stops it
+
