@@ -36,7 +36,7 @@ CHEB_ORDER, CHEB_NVEC, CHEB_LO, CHEB_HI = 64, 24, 0.01, 70.0
 CG_ITERS = 20
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (ncu --set full; average of the two
 # epilogue variants), filled in from the capture summarised in NCU_TRAFFIC_SOURCE
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 625.3e6
 NCU_TRAFFIC_SOURCE = "profiles/r1_10_cheb_tile.md"
 WORKLOAD = "16^3x32xLs16 fp32: D_hop/D_DW/H_DW/D_PV (nrhs 1,12,48) + Schur(4) + BLAS-1 + order-64 Chebyshev(24) + 20 rb-CG it"
 

@@ -621,7 +621,7 @@ static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nr
         else      inner_kernel<double, false><<<blocks, 256, 0, h->stream>>>((const double2*)x, (const double2*)y, ng, BS, nrhs, h->partial);
     }
     LAUNCH_CHECK(h);
-    reduce_final_kernel<<<1, 64, 0, h->stream>>>(h->partial, (int)blocks, nrhs, dev_out, ostride, ncomp);
+    reduce_final_kernel<<<nrhs, 256, 0, h->stream>>>(h->partial, (int)blocks, nrhs, dev_out, ostride, ncomp);
     LAUNCH_CHECK(h);
     return DWF_OK;
 }
@@ -683,13 +683,13 @@ static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, double tol_rel = 
     if (int rc = schur_op(h, false, x, w, tmp, 1)) return rc;
     if (int rc = schur_op(h, true, w, q, tmp, 1)) return rc;
     cg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, q, r, p, ng, h->partial); LAUNCH_CHECK(h);
-    reduce_final_kernel<<<1, 64, 0, st>>>(h->partial, (int)blocks, 1, hist, 1, 1); LAUNCH_CHECK(h);
+    reduce_final_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, 1, hist, 1, 1); LAUNCH_CHECK(h);
     for (int k = 0; k < iters; k++) {
         if (int rc = schur_op(h, false, p, w, tmp, 1)) return rc;
         if (int rc = schur_op(h, true, w, q, tmp, 1)) return rc;
         if (int rc = reduce_to(h, true, w, nullptr, 1, 1, pAp + k, 1, 1)) return rc;
         cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, hist + k, pAp + k, h->partial); LAUNCH_CHECK(h);
-        reduce_final_kernel<<<1, 64, 0, st>>>(h->partial, (int)blocks, 1, hist + k + 1, 1, 1); LAUNCH_CHECK(h);
+        reduce_final_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, 1, hist + k + 1, 1, 1); LAUNCH_CHECK(h);
         cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, hist + k + 1, hist + k); LAUNCH_CHECK(h);
         if (done) *done = k + 1;
         if (tol_rel > 0.0 && ((k + 1) % check_every == 0 || k + 1 == iters)) {      // stopping test: |r_k|^2 <= tol^2 |r_0|^2
