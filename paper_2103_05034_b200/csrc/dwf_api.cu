@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdint>
 #include <algorithm>
+#include <array>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -94,7 +95,23 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     std::vector<int> idx_of(V4);                                                // lex site -> index within its parity
     long long cnt[2] = {0, 0};
     int nb[4], nt[4]; for (int i = 0; i < 4; i++) { nb[i] = L[i] / B[i]; nt[i] = B[i] / T[i]; }
+    // Order of the lattice blocks: DWF_BLOCK_ORDER=morton walks them along a Z-order curve (neighbouring blocks in all four
+    // directions stay close in the order: shorter reuse distance in L2), default = lexicographic (x fastest).
+    std::vector<std::array<int, 4>> blocks;
     for (int bt = 0; bt < nb[3]; bt++) for (int bz = 0; bz < nb[2]; bz++) for (int by = 0; by < nb[1]; by++) for (int bx = 0; bx < nb[0]; bx++)
+        blocks.push_back({bx, by, bz, bt});
+    {
+        const char* ord = getenv("DWF_BLOCK_ORDER");
+        if (ord && !strcmp(ord, "morton")) {
+            auto code = [](const std::array<int, 4>& b) {
+                unsigned long long c = 0;
+                for (int bit = 0; bit < 16; bit++) for (int d = 0; d < 4; d++) c |= (unsigned long long)((b[d] >> bit) & 1) << (4 * bit + d);
+                return c;
+            };
+            std::stable_sort(blocks.begin(), blocks.end(), [&](const std::array<int, 4>& x, const std::array<int, 4>& y) { return code(x) < code(y); });
+        }
+    }
+    for (const auto& bb : blocks) { const int bx = bb[0], by = bb[1], bz = bb[2], bt = bb[3];
       for (int tt = 0; tt < nt[3]; tt++) for (int tz = 0; tz < nt[2]; tz++) for (int ty = 0; ty < nt[1]; ty++) for (int tx = 0; tx < nt[0]; tx++) {
         const int o[4] = {bx * B[0] + tx * T[0], by * B[1] + ty * T[1], bz * B[2] + tz * T[2], bt * B[3] + tt * T[3]};
         for (int t = o[3]; t < o[3] + T[3]; t++) for (int z = o[2]; z < o[2] + T[2]; z++)
@@ -106,6 +123,7 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
                 cnt[p]++;
             }
       }
+    }
     nbr.assign(2 * V4h * 8, 0);
     for (int p = 0; p < 2; p++) for (long long i = 0; i < V4h; i++) {
         long long lx = lex[p * V4h + i];
@@ -262,6 +280,8 @@ struct HopCall {            // precision-independent description of one launch
     const void* in_hop[2]; const void* in_self[2]; void* out[2]; const void* y[2]; const void* z[2];
     double c_hop, mass, ax_a, ax_b, ax_c;
     int nrhs;
+    double* norm_partial;   // tiled HM_HOP_SELF only: also write |out|^2 partials [item][warp][2] (nrhs = 1)
+    long long* norm_count;  // ... and return how many partials there are
 };
 
 template <typename R>
@@ -296,15 +316,17 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.glinks[0] = (const R*)h->glinks;
     a.glinks[1] = (const R*)((const char*)h->glinks + (size_t)h->V4h * lsite);
     a.sigma = (R)(-2.0 * k.c_hop);                                             // links carry the factor -1/2
+    a.norm_partial = k.norm_partial;
     {
         const double kappa = 1.0 / (5.0 - h->M5);
         a.moo_kappa = (R)kappa; a.moo_v0scale = (R)(kappa / (1.0 + k.mass * std::pow(kappa, (double)h->Ls)));
     }
     if (k.mode == HM_HOP_MOOINV && !TS) FAIL(h, DWF_EINVAL, "fused hop + M_oo^-1 needs the tiled kernel");
 #define HOPK(LS, DAG, HOP, SELF, G5, AX) hop_kernel<R, LS, DAG, HOP, SELF, G5, AX><<<grid, HOP_THREADS, 0, st>>>(a)
-#define TILEK(LS, TSV, DAG, SELF, G5, AX, MOO) do { \
+#define TILEK(LS, TSV, DAG, SELF, G5, AX, MOO, NRM) do { \
         using TG = TileGeom<R, LS, TSV>; \
-        auto kern = hop_tile_kernel<R, LS, TSV, DAG, true, SELF, G5, AX, MOO>; \
+        auto kern = hop_tile_kernel<R, LS, TSV, DAG, true, SELF, G5, AX, MOO, NRM>; \
+        if (NRM && k.norm_count) *k.norm_count = a.nitems * (TG::THREADS / 32); \
         cudaError_t e_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TG::SMEM_BYTES); \
         if (e_ != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e_)); \
         const long long ctas = std::min<long long>(a.nitems, (long long)h->sm_count * TG::MIN_CTAS); \
@@ -320,11 +342,13 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     }
 #define TILEM(LS, TSV) \
     switch (k.mode) { \
-        case HM_HOP:               if (k.dag) TILEK(LS, TSV, true, false, false, false, false); else TILEK(LS, TSV, false, false, false, false, false); break; \
-        case HM_HOP_MOOINV:        if (k.dag) TILEK(LS, TSV, true, false, false, false, true); else TILEK(LS, TSV, false, false, false, false, true); break; \
-        case HM_HOP_SELF:          if (k.dag) TILEK(LS, TSV, true, true, false, false, false);  else TILEK(LS, TSV, false, true, false, false, false); break; \
-        case HM_HOP_SELF_G5:       TILEK(LS, TSV, false, true, true, false, false); break; \
-        case HM_HOP_SELF_G5_AXPBY: TILEK(LS, TSV, false, true, true, true, false); break; \
+        case HM_HOP:               if (k.dag) TILEK(LS, TSV, true, false, false, false, false, false); else TILEK(LS, TSV, false, false, false, false, false, false); break; \
+        case HM_HOP_MOOINV:        if (k.dag) TILEK(LS, TSV, true, false, false, false, true, false); else TILEK(LS, TSV, false, false, false, false, true, false); break; \
+        case HM_HOP_SELF:          if (k.dag) TILEK(LS, TSV, true, true, false, false, false, false); \
+                                   else if (k.norm_partial) TILEK(LS, TSV, false, true, false, false, false, true); \
+                                   else TILEK(LS, TSV, false, true, false, false, false, false); break; \
+        case HM_HOP_SELF_G5:       TILEK(LS, TSV, false, true, true, false, false, false); break; \
+        case HM_HOP_SELF_G5_AXPBY: TILEK(LS, TSV, false, true, true, true, false, false); break; \
         default: FAIL(h, DWF_EINVAL, "bad hop mode"); \
     }
     // Right-hand sides are processed in chunks (one launch each) so that the working set of a chunk keeps
@@ -391,7 +415,9 @@ static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, co
 
 // Schur operator on even half fields:  tmp_o = M_oo^-1 Dhop_oe in ;
 // out = M_ee in - 1/4 Dhop_eo tmp_o     [M_eo = M_oe = -1/2 Dhop].  dag: every factor adjoint.
-static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs) {
+// norm_out != NULL (nrhs = 1, not dag): also *norm_out = |out|^2 on the device; fused into K2 when the tiled kernel applies.
+static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp);
+static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs, double* norm_out = nullptr) {
     // K1: tmp_o = M_oo^-1 Dhop_oe in -- one launch when the tiled kernel applies (M_oo^-1 fused as its epilogue)
     const bool fused = h->glinks && h->tile_sites && (h->Ls == 16 || h->Ls == 24) && !getenv("DWF_NO_FUSE_MOOINV");
     HopCall k1{};
@@ -402,7 +428,19 @@ static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, 
     HopCall k2{};
     k2.mode = HM_HOP_SELF; k2.dag = dag; k2.nslots = 1; k2.parity0 = 0; k2.nrhs = nrhs;
     k2.in_hop[0] = tmp; k2.in_self[0] = in; k2.out[0] = out; k2.c_hop = -0.25; k2.mass = h->mass;
-    return launch_hop(h, k2);
+    long long nparts = 0;
+    const long long max_parts = (long long)MAX_RED_BLOCKS * MAX_NRHS;
+    const long long tile_warps = h->tile_sites ? (h->V4h / h->tile_sites) * ((long long)h->tile_sites * h->Ls / vl(h) / 32) : 0;
+    const bool fuse_norm = norm_out && fused && nrhs == 1 && !dag && tile_warps <= max_parts && !getenv("DWF_NO_FUSE_NORM");
+    if (fuse_norm) { k2.norm_partial = h->partial; k2.norm_count = &nparts; }
+    if (int rc = launch_hop(h, k2)) return rc;
+    if (!norm_out) return DWF_OK;
+    if (fuse_norm && nparts > 0) {
+        reduce_final_kernel<<<1, 256, 0, h->stream>>>(h->partial, (int)nparts, 1, norm_out, 1, 1);
+        LAUNCH_CHECK(h);
+        return DWF_OK;
+    }
+    return reduce_to(h, true, out, nullptr, nrhs, 1, norm_out, 1, 1);
 }
 
 static int apply_checked(dwf_ctx* h, int op, const void* in, void* out, int nrhs) {
@@ -685,9 +723,8 @@ static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, double tol_rel = 
     cg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, q, r, p, ng, h->partial); LAUNCH_CHECK(h);
     reduce_final_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, 1, hist, 1, 1); LAUNCH_CHECK(h);
     for (int k = 0; k < iters; k++) {
-        if (int rc = schur_op(h, false, p, w, tmp, 1)) return rc;
+        if (int rc = schur_op(h, false, p, w, tmp, 1, pAp + k)) return rc;         // w = M p and <p, A p> = |w|^2
         if (int rc = schur_op(h, true, w, q, tmp, 1)) return rc;
-        if (int rc = reduce_to(h, true, w, nullptr, 1, 1, pAp + k, 1, 1)) return rc;
         cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, hist + k, pAp + k, h->partial); LAUNCH_CHECK(h);
         reduce_final_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, 1, hist + k + 1, 1, 1); LAUNCH_CHECK(h);
         cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, hist + k + 1, hist + k); LAUNCH_CHECK(h);

@@ -43,6 +43,7 @@ template <typename R> struct HopArgs {
     R sigma;               // res = sigma * hop' + self  with hop' built from the (-1/2)-scaled links
     R moo_kappa, moo_v0scale;   // fused M_oo^-1 epilogue: 1/(5-M5), kappa / (1 + m kappa^Ls)
     long long nitems;      // work items (tile, rhs, parity slot) of this launch
+    double* norm_partial;  // NORM epilogue: |out|^2 partials [item][warp][2]
     long long ngroups;     // ceil(V4h / G)
     long long chunk_groups;
     R c_hop, c_diag, mass;

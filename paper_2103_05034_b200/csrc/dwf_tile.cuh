@@ -14,6 +14,7 @@
 // global memory.  res = sigma * hop' + self with hop' built from the scaled links (sigma = 1 for
 // D_DW, H_DW, D_PV: no scaling pass).  The self term is computed first, while the copies land.
 #pragma once
+#include "dwf_aux.cuh"
 #include "dwf_hop.cuh"
 
 #ifndef DWF_INT_STAGES
@@ -107,7 +108,7 @@ __device__ __forceinline__ void tile_dir(CV<V> (&acc)[12], const G* psi, const i
     hop_dir_core<MU, SG, FWD>(acc, p, u);
 }
 
-template <typename R, int LS, int TS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY, bool MOO = false>
+template <typename R, int LS, int TS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY, bool MOO = false, bool NORM = false>
 __global__ void __launch_bounds__(TileGeom<R, LS, TS>::THREADS, TileGeom<R, LS, TS>::MIN_CTAS)
 hop_tile_kernel(const HopArgs<R> a) {
     static_assert(!MOO || (HOP && !SELF && !G5 && !AXPBY && TileGeom<R, LS, TS>::NSTI == 1), "fused M_oo^-1 follows a bare hop");
@@ -303,6 +304,19 @@ hop_tile_kernel(const HopArgs<R> a) {
         G* o = a.out[pi] + obase;
 #pragma unroll
         for (int c = 0; c < 12; c++) o[c * K] = pack(acc[c]);
+        if constexpr (NORM) {
+            // |out|^2 of this item, fp64: fixed shuffle tree inside the warp, one partial per (item, warp) at a fixed slot,
+            // summed later in slot order by reduce_final_kernel: deterministic whichever CTA ran the item.
+            double sre = 0, sim = 0;
+#pragma unroll
+            for (int c = 0; c < 12; c++) acc_inner(sre, sim, acc[c], acc[c]);
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) sre += __shfl_xor_sync(0xffffffffu, sre, off);
+            if ((threadIdx.x & 31) == 0) {
+                double* slot = a.norm_partial + ((size_t)w * NWARPS + (threadIdx.x >> 5)) * 2;
+                slot[0] = sre; slot[1] = 0.0;
+            }
+        }
     }
 }
 
