@@ -100,6 +100,13 @@ def dpv(U, psi, M5: float, dagger: bool = False) -> np.ndarray:
     return out
 
 
+def mpvdag_m(U, psi, M5: float, mass: float, dagger: bool = False) -> np.ndarray:
+    """Pauli-Villars preconditioned operator M_PV^dag M_l = D_PV^dag D_DW; dagger: D_DW^dag D_PV."""
+    if dagger:
+        return ddw(U, dpv(U, psi, M5), M5, mass, dagger=True)
+    return dpv(U, ddw(U, psi, M5, mass), M5, dagger=True)
+
+
 def gamma5r5(psi) -> np.ndarray:
     """Gamma5 psi = gamma5 R5 psi (L46)."""
     psi = _c(psi); L, Ls, nrhs = _geom(psi)

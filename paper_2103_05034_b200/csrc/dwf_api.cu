@@ -462,6 +462,11 @@ static int apply_checked(dwf_ctx* h, int op, const void* in, void* out, int nrhs
             return launch_hop(h, k);
         }
         case DWF_MOOINV: return launch_mooinv(h, in, out, nrhs, h->mass, dag);
+        case DWF_MPVDAG_M: {                                  // D_PV^dag D_DW (dag: D_DW^dag D_PV): two stencil launches through the workspace
+            if (int rc = need_ws(h, 2 * half_bytes(h, nrhs))) return rc;
+            if (int rc = full_op(h, HM_HOP_SELF, false, -0.5, dag ? 1.0 : h->mass, in, h->ws, nrhs)) return rc;
+            return full_op(h, HM_HOP_SELF, true, -0.5, dag ? h->mass : 1.0, h->ws, out, nrhs);
+        }
         default: FAIL(h, DWF_EINVAL, "unknown op %d", op);
     }
 }

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libdwf.so")
 
 DWF_F32, DWF_F64 = 0, 1
-DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV, DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV = range(7)
+DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV, DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV, DWF_MPVDAG_M = range(8)
 DWF_DAGGER = 0x100
 _HALF_OPS = (DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV)
 

@@ -226,3 +226,15 @@ def test_solve_red_black(oracle, prec, tol):
     assert rel_l2(oracle.ddw(rig.U, got, M5, mass), eta) < 30 * tol    # ... and the oracle's operator agrees
     assert rel_l2(got, psi_or) < 100 * tol
     assert np.array_equal(rig.canonical(en, 1), eta)
+
+
+# ------------------------------------------------------------------ Pauli-Villars preconditioned operator
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_mpvdag_m(oracle, prec):
+    from paper_2103_05034_b200 import DWF_MPVDAG_M
+    L, Ls, mass, nrhs = (4, 4, 6, 8), 8, 0.01, 2
+    rig = Rig(L, Ls, prec, mass, seed_U=1000, ws_nrhs=nrhs)
+    psi = rig.spinor(nrhs, 2010)
+    tol = 2 * TOL_APPLY[prec]                                         # two operator applies
+    assert rel_l2(rig.apply(DWF_MPVDAG_M, psi), oracle.mpvdag_m(rig.U, psi, M5, mass)) < tol
+    assert rel_l2(rig.apply(DWF_MPVDAG_M | DWF_DAGGER, psi), oracle.mpvdag_m(rig.U, psi, M5, mass, dagger=True)) < tol

@@ -250,3 +250,22 @@ def test_solve_rb_against_dense_solve(oracle):
     loose, it2 = oracle.solve_rb(U, eta, M5, MASS, 1e-3, 400)
     assert it2 < iters and 1e-7 < rel(oracle.ddw(U, loose, M5, MASS), eta) < 1e-1     # the tolerance is what stops it
 
+
+# ---------------------------------------------------------------- Pauli-Villars preconditioned operator (L101-107)
+def test_mpvdag_m_dense_and_half_plane(oracle):
+    """D_PV^dag D_DW against the dense product; and the property the paper quotes for it (L105): the half-plane condition,
+    i.e. the hermitian part of M_PV^dag M_l is positive definite (while D_DW itself is not: its hermitian part is indefinite... for
+    the squared operator the spectrum is real, for this one complex with positive real part)."""
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    x = gen.spinor_gaussian(L, Ls, 1, 12)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    Dpv = dense.ddw_5d(U, L, Ls, M5, 1.0)
+    A = Dpv.conj().T @ D
+    assert rel(oracle.mpvdag_m(U, x, M5, MASS)[0].reshape(-1), A @ x[0].reshape(-1)) < 1e-13
+    assert rel(oracle.mpvdag_m(U, x, M5, MASS, dagger=True)[0].reshape(-1), A.conj().T @ x[0].reshape(-1)) < 1e-13
+    herm = np.linalg.eigvalsh(0.5 * (A + A.conj().T))
+    assert herm[0] > 0                                              # half-plane condition
+    ev = np.linalg.eigvals(A)
+    assert ev.real.min() > 0 and np.abs(ev.imag).max() > 1e-3       # complex spectrum in the right half plane
+
