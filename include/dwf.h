@@ -52,6 +52,8 @@ enum { DWF_F32 = 0, DWF_F64 = 1 };
 enum { DWF_DHOP = 0, DWF_DDW = 1, DWF_HDW = 2, DWF_DPV = 3, DWF_SCHUR_EO = 4, DWF_MEE = 5, DWF_MOOINV = 6,
        DWF_MPVDAG_M = 7,   /* Pauli-Villars preconditioned operator D_PV^dag D_DW; full fields; uses the
                               workspace (1 full field); with DWF_DAGGER: D_DW^dag D_PV */
+       DWF_SCHUR_EO_ALT = 8, /* the other Schur form of Table V (L387): 1 - M_ee^-1 M_eo M_oo^-1 M_oe on EVEN half fields;
+                              uses the workspace (2 half fields); with DWF_DAGGER its adjoint */
        DWF_DAGGER = 0x100 };
 
 enum { DWF_OK = 0, DWF_EINVAL = -1, DWF_ENOGAUGE = -2, DWF_ENOMEM = -3, DWF_ECUDA = -4,

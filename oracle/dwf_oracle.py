@@ -156,6 +156,19 @@ def mpc(U, psi_e, M5: float, mass: float, dagger: bool = False) -> np.ndarray:
     return out
 
 
+def mpc_alt(U, psi_e, M5: float, mass: float, dagger: bool = False) -> np.ndarray:
+    """The other Schur form of Table V (L387): 1 - M_ee^-1 M_eo M_oo^-1 M_oe on an even half field, M_eo = M_oe = -1/2 Dhop
+    (eq. 4-5); dagger: the adjoint, factors reversed."""
+    psi = _c(psi_e)
+    if not dagger:
+        t = mpp_inv(-0.5 * dhop(U, psi, row_parity=1), M5, mass, 1)
+        return psi - mpp_inv(-0.5 * dhop(U, t, row_parity=0), M5, mass, 0)
+    # A^dag = 1 - M_oe^dag (M_oo^dag)^-1 M_eo^dag (M_ee^dag)^-1 ; (Dhop restricted to rows p)^dag maps parity p -> 1-p
+    t = mpp_inv(psi, M5, mass, 0, dagger=True)
+    t = mpp_inv(-0.5 * dhop(U, t, row_parity=0, dagger=True), M5, mass, 1, dagger=True)
+    return psi - (-0.5) * dhop(U, t, row_parity=1, dagger=True)
+
+
 def chebyshev(U, psi, M5: float, mass: float, order: int, lo: float, hi: float) -> np.ndarray:
     """T_order(2(D^dag D - lo)/(hi-lo) - 1) psi (eq. 23, eq. 34)."""
     psi = _c(psi); U = _c(U); L, Ls, nrhs = _geom(psi)

@@ -5,7 +5,7 @@ only: every step of the path runs in the library's kernels.  There is no CPU fal
 this package without the built library raises.
 """
 from .dwf import (Dwf, DwfError, DWF_F32, DWF_F64, DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV, DWF_SCHUR_EO,
-                  DWF_MEE, DWF_MOOINV, DWF_MPVDAG_M, DWF_DAGGER, lib_path, exported_symbols)
+                  DWF_MEE, DWF_MOOINV, DWF_MPVDAG_M, DWF_SCHUR_EO_ALT, DWF_DAGGER, lib_path, exported_symbols)
 
 __all__ = ["Dwf", "DwfError", "DWF_F32", "DWF_F64", "DWF_DHOP", "DWF_DDW", "DWF_HDW", "DWF_DPV",
-           "DWF_SCHUR_EO", "DWF_MEE", "DWF_MOOINV", "DWF_MPVDAG_M", "DWF_DAGGER", "lib_path", "exported_symbols"]
+           "DWF_SCHUR_EO", "DWF_MEE", "DWF_MOOINV", "DWF_MPVDAG_M", "DWF_SCHUR_EO_ALT", "DWF_DAGGER", "lib_path", "exported_symbols"]

@@ -462,6 +462,32 @@ static int apply_checked(dwf_ctx* h, int op, const void* in, void* out, int nrhs
             return launch_hop(h, k);
         }
         case DWF_MOOINV: return launch_mooinv(h, in, out, nrhs, h->mass, dag);
+        case DWF_SCHUR_EO_ALT: {                              // 1 - M_ee^-1 M_eo M_oo^-1 M_oe = 1 - 1/4 M_ee^-1 Dhop_eo M_oo^-1 Dhop_oe
+            // adjoint: 1 - 1/4 Dhop_oe^dag (M_oo^dag)^-1 Dhop_eo^dag (M_ee^dag)^-1  (the factors in reverse order)
+            const size_t hb = half_bytes(h, nrhs);
+            if (int rc = need_ws(h, 2 * hb)) return rc;
+            void* t1 = h->ws; void* t2 = (char*)h->ws + hb;
+            const bool fusedk = h->glinks && h->tile_sites && (h->Ls == 16 || h->Ls == 24) && !getenv("DWF_NO_FUSE_MOOINV");
+            auto hop_moo = [&](int parity_out, const void* src, void* dst, bool with_moo) -> int {   // dst_p = [M_pp^-1] Dhop src_{1-p}
+                HopCall k{}; k.mode = (with_moo && fusedk) ? HM_HOP_MOOINV : HM_HOP; k.dag = dag; k.nslots = 1; k.parity0 = parity_out; k.nrhs = nrhs;
+                k.in_hop[0] = src; k.out[0] = dst; k.c_hop = 1.0; k.mass = h->mass;
+                if (int rc = launch_hop(h, k)) return rc;
+                if (with_moo && !fusedk) return launch_mooinv(h, dst, dst, nrhs, h->mass, dag);
+                return DWF_OK;
+            };
+            if (!dag) {
+                if (int rc = hop_moo(1, in, t1, true)) return rc;                  // t1_o = M_oo^-1 Dhop_oe in
+                if (int rc = hop_moo(0, t1, t2, true)) return rc;                  // t2_e = M_ee^-1 Dhop_eo t1
+            } else {
+                if (int rc = launch_mooinv(h, in, t2, nrhs, h->mass, true)) return rc;   // t2_e = (M_ee^dag)^-1 in
+                if (int rc = hop_moo(1, t2, t1, true)) return rc;                  // t1_o = (M_oo^dag)^-1 Dhop_eo^dag t2   [Dhop_eo^dag maps even -> odd]
+                if (int rc = hop_moo(0, t1, t2, false)) return rc;                 // t2_e = Dhop_oe^dag t1
+            }
+            CUDA_TRY(h, cudaMemcpyAsync(out, in, hb, cudaMemcpyDeviceToDevice, h->stream));
+            double coef[2 * MAX_NRHS];
+            for (int q = 0; q < nrhs; q++) { coef[2 * q] = -0.25; coef[2 * q + 1] = 0.0; }
+            return dwf_axpy(h, coef, t2, out, nrhs, 1);
+        }
         case DWF_MPVDAG_M: {                                  // D_PV^dag D_DW (dag: D_DW^dag D_PV): two stencil launches through the workspace
             if (int rc = need_ws(h, 2 * half_bytes(h, nrhs))) return rc;
             if (int rc = full_op(h, HM_HOP_SELF, false, -0.5, dag ? 1.0 : h->mass, in, h->ws, nrhs)) return rc;
@@ -849,7 +875,7 @@ extern "C" int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* o
     if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
     if (!in_host || !out_host) FAIL(h, DWF_EINVAL, "NULL host pointer");
     const int base = op & ~DWF_DAGGER;
-    const bool halfop = (base == DWF_SCHUR_EO || base == DWF_MEE || base == DWF_MOOINV);
+    const bool halfop = (base == DWF_SCHUR_EO || base == DWF_MEE || base == DWF_MOOINV || base == DWF_SCHUR_EO_ALT);
     if (!halfop && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
     if (base == DWF_SCHUR_EO && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
     const size_t hb = half_bytes(h, nrhs), fb = 2 * hb;

@@ -16,9 +16,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libdwf.so")
 
 DWF_F32, DWF_F64 = 0, 1
-DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV, DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV, DWF_MPVDAG_M = range(8)
+DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV, DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV, DWF_MPVDAG_M, DWF_SCHUR_EO_ALT = range(9)
 DWF_DAGGER = 0x100
-_HALF_OPS = (DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV)
+_HALF_OPS = (DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV, DWF_SCHUR_EO_ALT)
 
 _SIGNATURES = {
     "dwf_create": (ctypes.c_int, [ctypes.POINTER(ctypes.c_int), ctypes.c_int, ctypes.c_double, ctypes.c_double,

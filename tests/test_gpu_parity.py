@@ -238,3 +238,16 @@ def test_mpvdag_m(oracle, prec):
     tol = 2 * TOL_APPLY[prec]                                         # two operator applies
     assert rel_l2(rig.apply(DWF_MPVDAG_M, psi), oracle.mpvdag_m(rig.U, psi, M5, mass)) < tol
     assert rel_l2(rig.apply(DWF_MPVDAG_M | DWF_DAGGER, psi), oracle.mpvdag_m(rig.U, psi, M5, mass, dagger=True)) < tol
+
+
+# ------------------------------------------------------------------ the other Schur form of Table V (L387; rest of N3)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("L,Ls", [((8, 8, 4, 4), 16), ((6, 4, 4, 8), 8)])          # tiled (fused M^-1) and generic path
+def test_schur_alt(oracle, prec, L, Ls):
+    from paper_2103_05034_b200 import DWF_SCHUR_EO_ALT
+    mass, nrhs = 0.02, 2
+    rig = Rig(L, Ls, prec, mass, seed_U=51, ws_nrhs=nrhs)
+    pe = gen.keep_parity(rig.spinor(nrhs, 52), L, 0)
+    tol = 2 * TOL_APPLY[prec]
+    assert rel_l2(rig.apply(DWF_SCHUR_EO_ALT, pe, half=True), oracle.mpc_alt(rig.U, pe, M5, mass)) < tol
+    assert rel_l2(rig.apply(DWF_SCHUR_EO_ALT | DWF_DAGGER, pe, half=True), oracle.mpc_alt(rig.U, pe, M5, mass, dagger=True)) < tol

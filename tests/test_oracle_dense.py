@@ -269,3 +269,24 @@ def test_mpvdag_m_dense_and_half_plane(oracle):
     ev = np.linalg.eigvals(A)
     assert ev.real.min() > 0 and np.abs(ev.imag).max() > 1e-3       # complex spectrum in the right half plane
 
+
+# ---------------------------------------------------------------- the other Schur form of Table V (L387)
+def test_mpc_alt_against_dense(oracle):
+    """1 - M_ee^-1 M_eo M_oo^-1 M_oe from the parity-partitioned dense D_DW; equals M_ee^-1 M_pc (the two forms of Table V
+    differ by the left factor M_ee^-1); adjoint = dense conjugate transpose."""
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    x = gen.keep_parity(gen.spinor_gaussian(L, Ls, 1, 13), L, 0)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    par = np.broadcast_to(gen.site_parity(L)[None, :, :, :, :, None, None], x[0].shape).reshape(-1)
+    e, o = np.where(par == 0)[0], np.where(par == 1)[0]
+    Mee, Meo, Moe, Moo = D[np.ix_(e, e)], D[np.ix_(e, o)], D[np.ix_(o, e)], D[np.ix_(o, o)]
+    A = np.eye(len(e)) - np.linalg.solve(Mee, Meo @ np.linalg.solve(Moo, Moe))
+    xe = x[0].reshape(-1)[e]
+    got = oracle.mpc_alt(U, x, M5, MASS)[0].reshape(-1)
+    assert rel(got[e], A @ xe) < 1e-12 and np.all(got[o] == 0)
+    gotd = oracle.mpc_alt(U, x, M5, MASS, dagger=True)[0].reshape(-1)
+    assert rel(gotd[e], A.conj().T @ xe) < 1e-12 and np.all(gotd[o] == 0)
+    mpc = oracle.mpc(U, x, M5, MASS)
+    assert rel(oracle.mpp_inv(mpc, M5, MASS, 0)[0].reshape(-1)[e], A @ xe) < 1e-12
+
