@@ -74,7 +74,8 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     int B[4] = {4, 4, 4, 4};      // outer block: unit of the parity interleave, L2 locality
     int T[4] = {4, 4, 2, 2};      // inner tile : 32 sites per parity = what one CTA of the tiled stencil works on
     // the tile interior of one rhs must fit shared memory twice per SM: 16-site tiles for wide blocks
-    if ((size_t)h->Ls * 96 * real_bytes(h) / 4 > 1536) T[1] = 2;
+    // (measured at 48^3x96 fp32 Ls 24: 32-site tiles x 1 CTA/SM 20.2 ms per apply, 16-site tiles x 2 CTAs/SM 24.2 ms)
+    if ((size_t)h->Ls * 24 * real_bytes(h) > 2304) T[1] = 2;
     auto parse = [](const char* name, int* v) {
         if (const char* env = getenv(name)) { int b[4]; if (sscanf(env, "%d,%d,%d,%d", &b[0], &b[1], &b[2], &b[3]) == 4) for (int i = 0; i < 4; i++) v[i] = b[i]; }
     };
@@ -284,6 +285,14 @@ struct HopCall {            // precision-independent description of one launch
     long long* norm_count;  // ... and return how many partials there are
 };
 
+// Is the tiled persistent stencil (dwf_tile.cuh) instantiated for this handle?  Lattice made of whole tiles, Ls 16 (16- or
+// 32-site tiles) or Ls 24 (16-site tiles; 32-site tiles in fp32), item index within 32 bits.
+static bool tiled_ok(const dwf_ctx* h) {
+    if (!h->glinks || !h->tile_sites) return false;
+    if (!(h->Ls == 16 || (h->Ls == 24 && (h->tile_sites == 16 || h->prec == DWF_F32)))) return false;
+    return 2 * (h->V4h / h->tile_sites + h->blk_sites) * (long long)h->rhs_chunk < (1LL << 31);
+}
+
 template <typename R>
 static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     using G = typename Prec<R>::G;
@@ -301,10 +310,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c;
     const int K = h->Ls / Prec<R>::VL;
     // tiled persistent stencil (dwf_tile.cuh): lattice made of whole tiles, compile-time Ls, a hop to do
-    const bool ls_ct = (h->Ls == 16 || h->Ls == 24);
-    // (its item index is 32-bit: fall back to the generic kernel for absurdly large launches)
-    const bool fits32 = h->tile_sites && 2 * (h->V4h / h->tile_sites + h->blk_sites) * (long long)h->rhs_chunk < (1LL << 31);
-    const int TS = (ls_ct && k.mode != HM_SELF && h->glinks && fits32) ? h->tile_sites : 0;
+    const int TS = (k.mode != HM_SELF && tiled_ok(h)) ? h->tile_sites : 0;
     a.sg_shift = h->sg_shift;
     a.GS = TS ? TS : std::min(HOP_THREADS / 8, HOP_THREADS / K);                                   // sites per CTA
     a.ngroups = (h->V4h + a.GS - 1) / a.GS;
@@ -360,7 +366,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
         dim3 grid((unsigned)(groups * a.rn));
         // compile-time Ls for the production sizes (tiled when the lattice allows), runtime Ls otherwise
         if (h->Ls == 16)      { if (TS == 32) { TILEM(16, 32) } else if (TS == 16) { TILEM(16, 16) } else { HOPM(16) } }
-        else if (h->Ls == 24) { if (TS == 16) { TILEM(24, 16) } else { HOPM(24) } }
+        else if (h->Ls == 24) { if (TS == 16) { TILEM(24, 16) } else if (TS == 32) { if constexpr (sizeof(R) == 4) { TILEM(24, 32) } } else { HOPM(24) } }
         else { HOPM(0) }
         LAUNCH_CHECK(h);
     }
@@ -419,7 +425,7 @@ static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, co
 static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp);
 static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs, double* norm_out = nullptr) {
     // K1: tmp_o = M_oo^-1 Dhop_oe in -- one launch when the tiled kernel applies (M_oo^-1 fused as its epilogue)
-    const bool fused = h->glinks && h->tile_sites && (h->Ls == 16 || h->Ls == 24) && !getenv("DWF_NO_FUSE_MOOINV");
+    const bool fused = tiled_ok(h) && !getenv("DWF_NO_FUSE_MOOINV");
     HopCall k1{};
     k1.mode = fused ? HM_HOP_MOOINV : HM_HOP; k1.dag = dag; k1.nslots = 1; k1.parity0 = 1; k1.nrhs = nrhs;
     k1.in_hop[0] = in; k1.out[0] = tmp; k1.c_hop = 1.0; k1.mass = h->mass;
@@ -467,7 +473,7 @@ static int apply_checked(dwf_ctx* h, int op, const void* in, void* out, int nrhs
             const size_t hb = half_bytes(h, nrhs);
             if (int rc = need_ws(h, 2 * hb)) return rc;
             void* t1 = h->ws; void* t2 = (char*)h->ws + hb;
-            const bool fusedk = h->glinks && h->tile_sites && (h->Ls == 16 || h->Ls == 24) && !getenv("DWF_NO_FUSE_MOOINV");
+            const bool fusedk = tiled_ok(h) && !getenv("DWF_NO_FUSE_MOOINV");
             auto hop_moo = [&](int parity_out, const void* src, void* dst, bool with_moo) -> int {   // dst_p = [M_pp^-1] Dhop src_{1-p}
                 HopCall k{}; k.mode = (with_moo && fusedk) ? HM_HOP_MOOINV : HM_HOP; k.dag = dag; k.nslots = 1; k.parity0 = parity_out; k.nrhs = nrhs;
                 k.in_hop[0] = src; k.out[0] = dst; k.c_hop = 1.0; k.mass = h->mass;
