@@ -89,8 +89,8 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     const int tsites = T[0] * T[1] * T[2] * T[3] / 2;
     bool whole = true;
     for (int i = 0; i < 4; i++) whole = whole && (L[i] % T[i] == 0);
-    h->tile_sites = (whole && (tsites == 16 || tsites == 32)) ? tsites : 0;
-    h->sg_shift = h->tile_sites == 32 ? 5 : h->tile_sites == 16 ? 4 : 0;
+    h->tile_sites = (whole && (tsites == 16 || tsites == 32 || tsites == 64)) ? tsites : 0;
+    h->sg_shift = h->tile_sites == 64 ? 6 : h->tile_sites == 32 ? 5 : h->tile_sites == 16 ? 4 : 0;
     if (getenv("DWF_NO_TILE")) h->tile_sites = 0;             // keeps the block order, uses the generic kernel
     lex.assign(2 * V4h, 0);
     std::vector<int> idx_of(V4);                                                // lex site -> index within its parity
@@ -289,6 +289,7 @@ struct HopCall {            // precision-independent description of one launch
 // 32-site tiles) or Ls 24 (16-site tiles; 32-site tiles in fp32), item index within 32 bits.
 static bool tiled_ok(const dwf_ctx* h) {
     if (!h->glinks || !h->tile_sites) return false;
+    if (h->tile_sites == 64 && !(h->Ls == 16 && h->prec == DWF_F32)) return false;
     if (!(h->Ls == 16 || (h->Ls == 24 && (h->tile_sites == 16 || h->prec == DWF_F32)))) return false;
     return 2 * (h->V4h / h->tile_sites + h->blk_sites) * (long long)h->rhs_chunk < (1LL << 31);
 }
@@ -365,7 +366,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
         a.nitems = groups * a.rn;
         dim3 grid((unsigned)(groups * a.rn));
         // compile-time Ls for the production sizes (tiled when the lattice allows), runtime Ls otherwise
-        if (h->Ls == 16)      { if (TS == 32) { TILEM(16, 32) } else if (TS == 16) { TILEM(16, 16) } else { HOPM(16) } }
+        if (h->Ls == 16)      { if (TS == 64) { if constexpr (sizeof(R) == 4) { TILEM(16, 64) } } else if (TS == 32) { TILEM(16, 32) } else if (TS == 16) { TILEM(16, 16) } else { HOPM(16) } }
         else if (h->Ls == 24) { if (TS == 16) { TILEM(24, 16) } else if (TS == 32) { if constexpr (sizeof(R) == 4) { TILEM(24, 32) } } else { HOPM(24) } }
         else { HOPM(0) }
         LAUNCH_CHECK(h);

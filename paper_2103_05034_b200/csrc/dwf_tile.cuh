@@ -116,7 +116,7 @@ hop_tile_kernel(const HopArgs<R> a) {
     using G = typename Prec<R>::G;
     using TG = TileGeom<R, LS, TS>;
     constexpr int K = TG::K, BS = TG::BS;
-    constexpr int SH = (TS == 32) ? 5 : 4;
+    constexpr int SH = (TS == 64) ? 6 : (TS == 32) ? 5 : 4;
     constexpr int LSITE = TileLinks<R>::SITE;
     extern __shared__ __align__(128) unsigned char smem[];
     constexpr int NSTI = TG::NSTI;
