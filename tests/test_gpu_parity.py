@@ -251,3 +251,20 @@ def test_schur_alt(oracle, prec, L, Ls):
     tol = 2 * TOL_APPLY[prec]
     assert rel_l2(rig.apply(DWF_SCHUR_EO_ALT, pe, half=True), oracle.mpc_alt(rig.U, pe, M5, mass)) < tol
     assert rel_l2(rig.apply(DWF_SCHUR_EO_ALT | DWF_DAGGER, pe, half=True), oracle.mpc_alt(rig.U, pe, M5, mass, dagger=True)) < tol
+
+
+# ------------------------------------------------------------------ maximum number of right-hand sides (64) through the tiled kernel
+def test_max_nrhs(oracle):
+    L, Ls, mass, nrhs = (4, 4, 4, 4), 16, 0.01, 64
+    rig = Rig(L, Ls, "f32", mass, seed_U=61, ws_nrhs=nrhs)
+    psi = rig.spinor(nrhs, 62)
+    got = rig.apply(DWF_HDW, psi)
+    for r in (0, 31, 63):
+        assert rel_l2(got[r:r + 1], oracle.hdw(rig.U, psi[r:r + 1], M5, mass)) < TOL_APPLY["f32"], r
+    pe = gen.keep_parity(psi, L, 0)
+    gs = rig.apply(DWF_SCHUR_EO, pe, half=True)
+    for r in (0, 63):
+        assert rel_l2(gs[r:r + 1], oracle.mpc(rig.U, pe[r:r + 1], M5, mass)) < TOL_APPLY["f32"], r
+    from paper_2103_05034_b200 import DwfError
+    with pytest.raises(DwfError):
+        rig.d.apply(DWF_HDW, rig.d.field(1), rig.d.field(1), 65)        # nrhs > 64: DWF_EINVAL
