@@ -138,6 +138,11 @@ int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs, int half)
  * iters+1 values |r_k|^2.  Uses the workspace (5 half fields).  Synchronises at the end only. */
 int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, double* resid2_hist_host);
 
+/* The same CG on nrhs right-hand sides in lock step (one independent CG per rhs: per-rhs alpha, beta; every kernel serves all
+ * of them).  b_even, x_even: even half fields of nrhs right-hand sides; resid2_hist_host (may be NULL): (iters+1) * nrhs
+ * values, [k][r] = |r_k|^2 of rhs r.  Uses the workspace (5 half fields of nrhs right-hand sides). */
+int dwf_cg_schur_multi(dwf_handle h, const void* b_even, void* x_even, int iters, int nrhs, double* resid2_hist_host);
+
 /* Complete red-black solve of D_DW psi = eta (Table V; eq. 9), nrhs = 1, full native fields:
  *   eta'_e = eta_e - M_eo M_oo^-1 eta_o;  CGNR on M_pc^dag M_pc psi_e = M_pc^dag eta'_e from psi_e = 0, stopped when
  *   |r_k| <= tol |r_0| (r = residual of the normal equations; tested every 10 iterations) or after max_iters;

@@ -747,29 +747,31 @@ extern "C" int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs
 // <p_k, A p_k> = |M p_k|^2 at scal[iters+1+k].
 // ------------------------------------------------------------------------------------------------
 template <typename R>
-static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, double tol_rel = 0.0, int check_every = 10, int* done = nullptr) {
+static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, int nrhs = 1, double tol_rel = 0.0, int check_every = 10, int* done = nullptr) {
     using G = typename Prec<R>::G;
-    const size_t hb = half_bytes(h, 1);
-    const long long ng = half_groups(h, 1);
+    const size_t hb = half_bytes(h, nrhs);
+    const long long ng = half_groups(h, nrhs);
+    const int BS = run_groups(h);
     G* r = (G*)h->ws; G* p = (G*)((char*)h->ws + hb); G* w = (G*)((char*)h->ws + 2 * hb);
     G* q = (G*)((char*)h->ws + 3 * hb); void* tmp = (char*)h->ws + 4 * hb;
-    double* hist = h->scal; double* pAp = h->scal + iters + 1;
-    const unsigned blocks = (unsigned)std::min<long long>((ng + 255) / 256, std::min<long long>((long long)h->sm_count * 8, MAX_RED_BLOCKS));
+    double* hist = h->scal; double* pAp = h->scal + (size_t)(iters + 1) * nrhs;     // hist[k*nrhs + r], pAp[k*nrhs + r]
+    const unsigned blocks = blas_blocks(h, ng, (long long)BS * nrhs);
     cudaStream_t st = h->stream;
-    if (int rc = schur_op(h, false, x, w, tmp, 1)) return rc;
-    if (int rc = schur_op(h, true, w, q, tmp, 1)) return rc;
-    cg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, q, r, p, ng, h->partial); LAUNCH_CHECK(h);
-    reduce_final_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, 1, hist, 1, 1); LAUNCH_CHECK(h);
+    if (int rc = schur_op(h, false, x, w, tmp, nrhs)) return rc;
+    if (int rc = schur_op(h, true, w, q, tmp, nrhs)) return rc;
+    cg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, q, r, p, ng, BS, nrhs, h->partial); LAUNCH_CHECK(h);
+    reduce_final_kernel<<<nrhs, 256, 0, st>>>(h->partial, (int)blocks, nrhs, hist, 1, 1); LAUNCH_CHECK(h);
     for (int k = 0; k < iters; k++) {
-        if (int rc = schur_op(h, false, p, w, tmp, 1, pAp + k)) return rc;         // w = M p and <p, A p> = |w|^2
-        if (int rc = schur_op(h, true, w, q, tmp, 1)) return rc;
-        cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, hist + k, pAp + k, h->partial); LAUNCH_CHECK(h);
-        reduce_final_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, 1, hist + k + 1, 1, 1); LAUNCH_CHECK(h);
-        cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, hist + k + 1, hist + k); LAUNCH_CHECK(h);
+        double* hk = hist + (size_t)k * nrhs; double* hk1 = hk + nrhs; double* pk = pAp + (size_t)k * nrhs;
+        if (int rc = schur_op(h, false, p, w, tmp, nrhs, pk)) return rc;           // w = M p and <p, A p> = |w|^2
+        if (int rc = schur_op(h, true, w, q, tmp, nrhs)) return rc;
+        cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, BS, nrhs, hk, pk, h->partial); LAUNCH_CHECK(h);
+        reduce_final_kernel<<<nrhs, 256, 0, st>>>(h->partial, (int)blocks, nrhs, hk1, 1, 1); LAUNCH_CHECK(h);
+        cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, BS, nrhs, hk1, hk); LAUNCH_CHECK(h);
         if (done) *done = k + 1;
-        if (tol_rel > 0.0 && ((k + 1) % check_every == 0 || k + 1 == iters)) {      // stopping test: |r_k|^2 <= tol^2 |r_0|^2
+        if (tol_rel > 0.0 && ((k + 1) % check_every == 0 || k + 1 == iters)) {      // stopping test (nrhs = 1): |r_k|^2 <= tol^2 |r_0|^2
             CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, hist, sizeof(double), cudaMemcpyDeviceToHost, st));
-            CUDA_TRY(h, cudaMemcpyAsync(h->scal_host + 1, hist + k + 1, sizeof(double), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(h, cudaMemcpyAsync(h->scal_host + 1, hk1, sizeof(double), cudaMemcpyDeviceToHost, st));
             CUDA_TRY(h, cudaStreamSynchronize(st));
             if (h->scal_host[1] <= tol_rel * tol_rel * h->scal_host[0]) break;
         }
@@ -777,14 +779,15 @@ static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, double tol_rel = 
     return DWF_OK;
 }
 
-extern "C" int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, double* hist_host) {
+static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int iters, int nrhs, double* hist_host) {
     if (!h) return DWF_EINVAL;
-    if (iters < 0 || 2 * iters + 2 > SCAL_DOUBLES) FAIL(h, DWF_EINVAL, "iters out of range");
+    if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
+    if (iters < 0 || 2 * (long long)(iters + 1) * nrhs > SCAL_DOUBLES) FAIL(h, DWF_EINVAL, "iters out of range");
     if (int rc = check_field(h, b_even, "b_even")) return rc;
     if (int rc = check_field(h, x_even, "x_even")) return rc;
     if (b_even == x_even) FAIL(h, DWF_EINVAL, "b == x");
     if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
-    if (int rc = need_ws(h, 5 * half_bytes(h, 1))) return rc;
+    if (int rc = need_ws(h, 5 * half_bytes(h, nrhs))) return rc;
     // The host loop only enqueues (alpha, beta live on the device).  DWF_CG_GRAPH=1 captures the whole solve into a
     // CUDA graph and launches it as one unit; measured on B200 (8^4x16: 7037 vs 7388 it/s, 16^3x32x16: no change)
     // the plain stream launches are already back to back, so the graph is off by default.
@@ -796,7 +799,7 @@ extern "C" int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int 
         cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
         CUDA_TRY(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
         h->stream = h->cap_stream;
-        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters) : cg_t<double>(h, b_even, x_even, iters);
+        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs) : cg_t<double>(h, b_even, x_even, iters, nrhs);
         h->stream = user;
         cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
         if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -808,13 +811,21 @@ extern "C" int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int 
         cudaGraphDestroy(graph);
         if (e != cudaSuccess) FAIL(h, DWF_ECUDA, "CUDA graph of the CG loop: %s", cudaGetErrorString(e));
     } else {
-        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters) : cg_t<double>(h, b_even, x_even, iters);
+        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs) : cg_t<double>(h, b_even, x_even, iters, nrhs);
         if (rc) return rc;
     }
-    CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, (iters + 1) * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    const size_t nh = (size_t)(iters + 1) * nrhs;
+    CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, nh * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    if (hist_host) memcpy(hist_host, h->scal_host, (iters + 1) * sizeof(double));
+    if (hist_host) memcpy(hist_host, h->scal_host, nh * sizeof(double));
     return DWF_OK;
+}
+
+extern "C" int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, double* hist_host) {
+    return cg_schur_impl(h, b_even, x_even, iters, 1, hist_host);
+}
+extern "C" int dwf_cg_schur_multi(dwf_handle h, const void* b_even, void* x_even, int iters, int nrhs, double* hist_host) {
+    return cg_schur_impl(h, b_even, x_even, iters, nrhs, hist_host);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -850,7 +861,7 @@ extern "C" int dwf_solve(dwf_handle h, const void* eta, void* psi, double tol, i
     // CGNR from x_0 = 0
     CUDA_TRY(h, cudaMemsetAsync(psi_e, 0, hb, h->stream));
     int done = 0;
-    int rc = h->prec == DWF_F32 ? cg_t<float>(h, B, psi_e, max_iters, tol, 10, &done) : cg_t<double>(h, B, psi_e, max_iters, tol, 10, &done);
+    int rc = h->prec == DWF_F32 ? cg_t<float>(h, B, psi_e, max_iters, 1, tol, 10, &done) : cg_t<double>(h, B, psi_e, max_iters, 1, tol, 10, &done);
     if (rc) return rc;
     // reconstruction of the odd sites
     if (int rc2 = hop_to(1, psi_e, W)) return rc2;

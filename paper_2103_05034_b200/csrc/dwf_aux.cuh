@@ -218,36 +218,41 @@ reduce_final_kernel(const double* __restrict__ partial, int nblocks, int nrhs, d
 }
 
 // ------------------------------------------------------------------------------------------------
-// a9. CG vector updates (nrhs = 1, half fields), scalars read from device memory:
+// a9. CG vector updates (half fields, nrhs right-hand sides: one CG per rhs in lock step), scalars read from device
+// memory, one per rhs; launch geometry as for BLAS-1 (a thread keeps one rhs):
 //   init  : r = b - q ; p = r ;                              partial |r|^2
-//   xr    : alpha = rr[0] / pAp[0] ; x += alpha p ; r -= alpha q ; partial |r|^2
-//   p     : beta  = rr_new[0] / rr_old[0] ; p = r + beta p
+//   xr    : alpha = rr[r] / pAp[r] ; x += alpha p ; r -= alpha q ; partial |r|^2
+//   p     : beta  = rr_new[r] / rr_old[r] ; p = r + beta p
 // ------------------------------------------------------------------------------------------------
 template <typename R>
 __global__ void __launch_bounds__(256)
 cg_init_kernel(const typename Prec<R>::G* __restrict__ b, const typename Prec<R>::G* __restrict__ q,
-               typename Prec<R>::G* r, typename Prec<R>::G* p, long long ngroups, double* partial) {
+               typename Prec<R>::G* r, typename Prec<R>::G* p, long long ngroups, int BS, int nrhs, double* partial) {
     using V = typename Prec<R>::V;
     const long long stride = (long long)gridDim.x * blockDim.x;
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int rhs = (int)((e / BS) % nrhs);
     double sre = 0, sim = 0;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+    for (; e < ngroups; e += stride) {
         const CV<V> rr = csub(unpack(ldg_nc(b + e)), unpack(ldg_nc(q + e)));
         r[e] = pack(rr); p[e] = pack(rr);
         acc_inner(sre, sim, rr, rr);
     }
-    block_combine(sre, sim, 0, 1, partial);
+    block_combine(sre, sim, rhs, nrhs, partial);
 }
 
 template <typename R>
 __global__ void __launch_bounds__(256)
 cg_update_xr_kernel(typename Prec<R>::G* x, typename Prec<R>::G* r, const typename Prec<R>::G* __restrict__ p,
-                    const typename Prec<R>::G* __restrict__ q, long long ngroups,
+                    const typename Prec<R>::G* __restrict__ q, long long ngroups, int BS, int nrhs,
                     const double* __restrict__ rr, const double* __restrict__ pAp, double* partial) {
     using V = typename Prec<R>::V;
-    const R alpha = (R)(rr[0] / pAp[0]);
     const long long stride = (long long)gridDim.x * blockDim.x;
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int rhs = (int)((e / BS) % nrhs);
+    const R alpha = (R)(rr[rhs] / pAp[rhs]);
     double sre = 0, sim = 0;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+    for (; e < ngroups; e += stride) {
         const CV<V> pp = unpack(ldg_nc(p + e)), qq = unpack(ldg_nc(q + e));
         CV<V> xx = unpack(x[e]), rv = unpack(r[e]);
         xx.re = vfma(alpha, pp.re, xx.re); xx.im = vfma(alpha, pp.im, xx.im);
@@ -255,17 +260,19 @@ cg_update_xr_kernel(typename Prec<R>::G* x, typename Prec<R>::G* r, const typena
         x[e] = pack(xx); r[e] = pack(rv);
         acc_inner(sre, sim, rv, rv);
     }
-    block_combine(sre, sim, 0, 1, partial);
+    block_combine(sre, sim, rhs, nrhs, partial);
 }
 
 template <typename R>
 __global__ void __launch_bounds__(256)
-cg_update_p_kernel(typename Prec<R>::G* p, const typename Prec<R>::G* __restrict__ r, long long ngroups,
+cg_update_p_kernel(typename Prec<R>::G* p, const typename Prec<R>::G* __restrict__ r, long long ngroups, int BS, int nrhs,
                    const double* __restrict__ rr_new, const double* __restrict__ rr_old) {
     using V = typename Prec<R>::V;
-    const R beta = (R)(rr_new[0] / rr_old[0]);
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int rhs = (int)((e / BS) % nrhs);
+    const R beta = (R)(rr_new[rhs] / rr_old[rhs]);
+    for (; e < ngroups; e += stride) {
         const CV<V> rv = unpack(ldg_nc(r + e));
         CV<V> pp = unpack(p[e]);
         pp.re = vfma(beta, pp.re, rv.re); pp.im = vfma(beta, pp.im, rv.im);

@@ -49,6 +49,8 @@ _SIGNATURES = {
                                  ctypes.c_int]),
     "dwf_cg_schur": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
                                     ctypes.POINTER(ctypes.c_double)]),
+    "dwf_cg_schur_multi": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
+                                          ctypes.POINTER(ctypes.c_double)]),
     "dwf_solve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_int,
                                  ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]),
     "dwf_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
@@ -229,6 +231,12 @@ class Dwf:
         hist = (ctypes.c_double * (iters + 1))()
         self._check(self.lib.dwf_cg_schur(self._h, ctypes.c_void_p(b_even.data_ptr()), ctypes.c_void_p(x_even.data_ptr()), iters, hist))
         return [float(v) for v in hist]
+
+    def cg_schur_multi(self, b_even: torch.Tensor, x_even: torch.Tensor, iters: int, nrhs: int):
+        """Returns the history as a list of (iters+1) lists of nrhs values."""
+        hist = (ctypes.c_double * ((iters + 1) * nrhs))()
+        self._check(self.lib.dwf_cg_schur_multi(self._h, ctypes.c_void_p(b_even.data_ptr()), ctypes.c_void_p(x_even.data_ptr()), iters, nrhs, hist))
+        return [[float(hist[k * nrhs + r]) for r in range(nrhs)] for k in range(iters + 1)]
 
     def solve(self, eta: torch.Tensor, psi: torch.Tensor, tol: float, max_iters: int):
         """D_DW psi = eta by the complete red-black CGNR solve; returns (iterations, true relative residual)."""

@@ -268,3 +268,24 @@ def test_max_nrhs(oracle):
     from paper_2103_05034_b200 import DwfError
     with pytest.raises(DwfError):
         rig.d.apply(DWF_HDW, rig.d.field(1), rig.d.field(1), 65)        # nrhs > 64: DWF_EINVAL
+
+
+# ------------------------------------------------------------------ multi-RHS CG (rest of SURVEY 8(f) N3): one CG per rhs in lock step
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_cg_multi_rhs(oracle, prec):
+    L, Ls, mass, nrhs, iters = (8, 4, 4, 8), 16, 0.01, 3, 25
+    rig = Rig(L, Ls, prec, mass, seed_U=71, ws_nrhs=nrhs)
+    b = gen.keep_parity(rig.spinor(nrhs, 72), L, 0)
+    bn = rig.native(b, 0)
+    xn = rig.d.field(nrhs, half=True, zero=True)
+    hist = np.array(rig.d.cg_schur_multi(bn, xn, iters, nrhs))          # [iters+1][nrhs]
+    x = rig.canonical(xn, nrhs, 0)
+    tol_h, tol_x = (1e-9, 1e-10) if prec == "f64" else (1e-4, 1e-5)
+    for r in range(nrhs):
+        x_or, h_or = oracle.cg_schur(rig.U, b[r:r + 1], M5, mass, iters)
+        assert np.max(np.abs(hist[:, r] - h_or) / h_or) < tol_h, r
+        assert rel_l2(x[r:r + 1], x_or) < tol_x, r
+    # nrhs = 1 through the multi entry point is the single-rhs solver
+    x1 = rig.d.field(1, half=True, zero=True)
+    h1 = rig.d.cg_schur(rig.native(b[0:1], 0), x1, iters)
+    assert np.max(np.abs(np.array(h1) - hist[:, 0]) / hist[:, 0]) < (1e-12 if prec == "f64" else 1e-5)
