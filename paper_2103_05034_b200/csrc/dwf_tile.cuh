@@ -303,7 +303,7 @@ hop_tile_kernel(const HopArgs<R> a) {
         }
         G* o = a.out[pi] + obase;
 #pragma unroll
-        for (int c = 0; c < 12; c++) o[c * K] = pack(acc[c]);
+        for (int c = 0; c < 12; c++) __stcs(o + c * K, pack(acc[c]));          // streaming store: the output is not re-read by this launch
         if constexpr (NORM) {
             // |out|^2 of this item, fp64: fixed shuffle tree inside the warp, one partial per (item, warp) at a fixed slot,
             // summed later in slot order by reduce_final_kernel: deterministic whichever CTA ran the item.
