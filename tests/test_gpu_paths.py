@@ -62,3 +62,27 @@ def test_cg_graph_vs_stream(monkeypatch):
     x2 = rig.d.field(1, half=True, zero=True)
     h2 = rig.d.cg_schur(b, x2, 20)
     assert h1 == h2 and bool((x1 == x2).all())        # deterministic reductions: bit identical
+
+
+@pytest.mark.parametrize("prec", ["f32", "f64"])
+def test_repeatable_bit_for_bit(prec):
+    """The persistent kernel hands its shared-memory buffers over through mbarriers and an atomic counter: a race there would
+    show up as run-to-run differences.  30 applies of H_DW (+ the Chebyshev pair, + the fused Schur) on one input at a size with
+    many work items per CTA must be bit identical."""
+    import torch
+    from paper_2103_05034_b200 import DWF_SCHUR_EO
+    L, Ls, nrhs = (16, 16, 8, 8), 16, 2
+    rig = Rig(L, Ls, prec, 0.01, seed_U=81, ws_nrhs=nrhs)
+    g = torch.Generator(device="cuda"); g.manual_seed(82)
+    x = rig.d.field(nrhs).normal_(generator=g)
+    ref_h, ref_c, ref_s = rig.d.field(nrhs), rig.d.field(nrhs), rig.d.field(nrhs, half=True)
+    rig.d.apply(DWF_HDW, x, ref_h, nrhs)
+    rig.d.chebyshev(3, 0.01, 70.0, x, ref_c, nrhs)
+    xe = x[: ref_s.numel()].clone()
+    rig.d.apply(DWF_SCHUR_EO, xe, ref_s, nrhs)
+    for _ in range(30):
+        y, c, s = rig.d.field(nrhs), rig.d.field(nrhs), rig.d.field(nrhs, half=True)
+        rig.d.apply(DWF_HDW, x, y, nrhs)
+        rig.d.chebyshev(3, 0.01, 70.0, x, c, nrhs)
+        rig.d.apply(DWF_SCHUR_EO, xe, s, nrhs)
+        assert torch.equal(y, ref_h) and torch.equal(c, ref_c) and torch.equal(s, ref_s)
