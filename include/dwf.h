@@ -151,6 +151,19 @@ int dwf_cg_schur_multi(dwf_handle h, const void* b_even, void* x_even, int iters
  * full-lattice operator.  eta != psi.  Uses the workspace (8 half fields).  Synchronises. */
 int dwf_solve(dwf_handle h, const void* eta, void* psi, double tol, int max_iters, int* iters_host, double* relres_host);
 
+/* Convert a full native field of nrhs right-hand sides from the precision (and site order) of handle `src` to that of
+ * handle `dst`: same lattice and Ls.  Enqueued on dst's stream. */
+int dwf_convert(dwf_handle src, dwf_handle dst, const void* in_native_src, void* out_native_dst, int nrhs);
+
+/* Mixed-precision solve of D_DW psi = eta ("single and mixed precision"; the usual defect correction):
+ *   repeat: r = eta - D_DW psi in fp64 (h64); stop when |r| <= tol |eta| or after max_outer corrections;
+ *           e = dwf_solve(h32, r, inner_tol, max_inner) in fp32; psi += e in fp64.
+ * h64 / h32: an fp64 and an fp32 handle with the same lattice, Ls, M5, mass, both with gauge and workspace
+ * (dwf_workspace_bytes(h, 1)) set and on the same stream.  eta, psi: fp64 full native fields of h64, nrhs = 1.
+ * *outer_host = corrections done, *inner_total_host = fp32 CG iterations in total, *relres_host = final |r|/|eta| (fp64). */
+int dwf_solve_mixed(dwf_handle h64, dwf_handle h32, const void* eta, void* psi, double tol, double inner_tol,
+                    int max_outer, int max_inner, int* outer_host, int* inner_total_host, double* relres_host);
+
 /* Number of kernel launches this handle has enqueued so far (for bench.py's gpu_launches). */
 long long dwf_launch_count(dwf_handle h);
 

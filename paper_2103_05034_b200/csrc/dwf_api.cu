@@ -29,6 +29,7 @@ struct dwf_ctx {
     void* glinks;         // gathered, (-1/2)-scaled links for the tiled stencil (tile_sites != 0)
     int* nbr;             // [2][V4h][8]
     int* lex;             // [2][V4h]
+    int* inv_lex;         // [V4]: lexicographic site -> index within its parity (built on first use by dwf_convert)
     bool have_gauge;
     void* ws; size_t ws_bytes;
     double* partial;      // reduction partials [MAX_RED_BLOCKS][64][2]
@@ -183,7 +184,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
 
 extern "C" int dwf_destroy(dwf_handle h) {
     if (!h) return DWF_EINVAL;
-    cudaFree(h->gauge); cudaFree(h->glinks); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal);
+    cudaFree(h->gauge); cudaFree(h->glinks); cudaFree(h->inv_lex); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal);
     if (h->scal_host) cudaFreeHost(h->scal_host);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     delete h;
@@ -200,7 +201,7 @@ extern "C" size_t dwf_field_bytes(dwf_handle h, int nrhs, int half) {
 }
 extern "C" size_t dwf_workspace_bytes(dwf_handle h, int nrhs) {
     if (!h || nrhs < 1) return 0;
-    return 8 * half_bytes(h, nrhs) + 256;          // dwf_chebyshev_smoother: 4 full fields
+    return 12 * half_bytes(h, nrhs) + 256;         // dwf_solve_mixed: 8 (dwf_solve) + 2 full fields
 }
 extern "C" int dwf_set_workspace(dwf_handle h, void* p, size_t n) {
     if (!h) return DWF_EINVAL;
@@ -881,6 +882,89 @@ extern "C" int dwf_solve(dwf_handle h, const void* eta, void* psi, double tol, i
     }
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (iters_host) *iters_host = done;
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Precision conversion between two handles on the same lattice, and the mixed-precision solve built on it
+// ("single and mixed precision").
+// ------------------------------------------------------------------------------------------------
+extern "C" int dwf_convert(dwf_handle src, dwf_handle dst, const void* in, void* out, int nrhs) {
+    if (!src || !dst) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(dst, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
+    for (int i = 0; i < 4; i++) if (src->L[i] != dst->L[i]) FAIL(dst, DWF_EINVAL, "dwf_convert: different lattices");
+    if (src->Ls != dst->Ls) FAIL(dst, DWF_EINVAL, "dwf_convert: different Ls");
+    if (int rc = check_field(dst, in, "in")) return rc;
+    if (int rc = check_field(dst, out, "out")) return rc;
+    cudaStream_t st = dst->stream;
+    if (!src->inv_lex) {
+        CUDA_TRY(dst, cudaMalloc((void**)&src->inv_lex, (size_t)src->V4 * sizeof(int)));
+        invert_lex_kernel<<<(unsigned)((2 * src->V4h + 255) / 256), 256, 0, st>>>(src->lex, src->inv_lex, src->V4h);
+        LAUNCH_CHECK(dst);
+    }
+    const long long total = 2 * src->V4h * nrhs * 12 * (src->Ls / 2);
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+#define CONV(RS, RD) convert_kernel<RS, RD><<<blocks, 256, 0, st>>>((const Prec<RS>::G*)in, (Prec<RD>::G*)out, src->inv_lex, dst->lex, \
+                                                                    src->V4h, src->Ls, nrhs, src->sg_shift, dst->sg_shift, 2)
+    if (src->prec == DWF_F64 && dst->prec == DWF_F32) CONV(double, float);
+    else if (src->prec == DWF_F32 && dst->prec == DWF_F64) CONV(float, double);
+    else if (src->prec == DWF_F32) CONV(float, float);
+    else CONV(double, double);
+#undef CONV
+    LAUNCH_CHECK(dst);
+    return DWF_OK;
+}
+
+// D_DW psi = eta to fp64 accuracy with the work done in fp32: defect correction
+//   r = eta - D psi (fp64);  e = dwf_solve(h32, r, inner_tol) (fp32 red-black CGNR);  psi += e (fp64);  until |r| <= tol |eta|.
+// Both handles: same lattice, Ls, M5, mass, gauge set (the fp32 one with the fp64 links rounded once), workspaces set
+// (dwf_workspace_bytes(h, 1) each), same stream.
+extern "C" int dwf_solve_mixed(dwf_handle h64, dwf_handle h32, const void* eta, void* psi, double tol, double inner_tol,
+                               int max_outer, int max_inner, int* outer_host, int* inner_total_host, double* relres_host) {
+    if (!h64 || !h32) return DWF_EINVAL;
+    if (h64->prec != DWF_F64 || h32->prec != DWF_F32) FAIL(h64, DWF_EINVAL, "dwf_solve_mixed needs an fp64 and an fp32 handle");
+    if (!(tol > 0.0) || !(inner_tol > 0.0) || max_outer < 1 || max_inner < 1) FAIL(h64, DWF_EINVAL, "bad tolerances / iteration limits");
+    if (h64->M5 != h32->M5 || h64->mass != h32->mass) FAIL(h64, DWF_EINVAL, "the two handles differ in M5 or mass");
+    if (int rc = check_field(h64, eta, "eta")) return rc;
+    if (int rc = check_field(h64, psi, "psi")) return rc;
+    if (eta == psi) FAIL(h64, DWF_EINVAL, "eta == psi");
+    if (!h64->have_gauge || !h32->have_gauge) FAIL(h64, DWF_ENOGAUGE, "dwf_set_gauge has not been called on both handles");
+    const size_t hb64 = half_bytes(h64, 1), hb32 = half_bytes(h32, 1);
+    if (int rc = need_ws(h64, 6 * hb64)) return rc;
+    if (need_ws(h32, 12 * hb32)) FAIL(h64, DWF_ENOWORKSPACE, "fp32 handle: workspace of %zu bytes needed", 12 * hb32);
+    char* Dpsi = (char*)h64->ws; char* r64 = Dpsi + 2 * hb64; char* e64 = Dpsi + 4 * hb64;
+    char* r32 = (char*)h32->ws + 8 * hb32; char* e32 = (char*)h32->ws + 10 * hb32;
+    const double one[2] = {1.0, 0.0}, minus[2] = {-1.0, 0.0};
+    double neta = 0, nr = 0;
+    if (int rc = dwf_norm2(h64, eta, &neta, 1, 0)) return rc;
+    if (!(neta > 0.0)) FAIL(h64, DWF_EINVAL, "eta is zero");
+    CUDA_TRY(h64, cudaMemsetAsync(psi, 0, 2 * hb64, h64->stream));
+    int outer = 0, inner_total = 0;
+    double rel = 1.0;
+    for (;;) {
+        // r = eta - D psi
+        if (outer == 0) CUDA_TRY(h64, cudaMemcpyAsync(r64, eta, 2 * hb64, cudaMemcpyDeviceToDevice, h64->stream));
+        else {
+            if (int rc = full_op(h64, HM_HOP_SELF, false, -0.5, h64->mass, psi, Dpsi, 1)) return rc;
+            CUDA_TRY(h64, cudaMemcpyAsync(r64, eta, 2 * hb64, cudaMemcpyDeviceToDevice, h64->stream));
+            if (int rc = dwf_axpy(h64, minus, Dpsi, r64, 1, 0)) return rc;
+        }
+        if (int rc = dwf_norm2(h64, r64, &nr, 1, 0)) return rc;
+        rel = std::sqrt(nr / neta);
+        if (rel <= tol || outer == max_outer) break;
+        // inner solve in fp32 on the residual (floating point: its relative accuracy does not depend on the size of r)
+        if (int rc = dwf_convert(h64, h32, r64, r32, 1)) return rc;
+        int it = 0;
+        if (int rc = dwf_solve(h32, r32, e32, inner_tol, max_inner, &it, nullptr)) { snprintf(h64->err, sizeof(h64->err), "inner solve: %.200s", h32->err); return rc; }
+        inner_total += it;
+        if (int rc = dwf_convert(h32, h64, e32, e64, 1)) return rc;
+        if (int rc = dwf_axpy(h64, one, e64, psi, 1, 0)) return rc;
+        outer++;
+    }
+    CUDA_TRY(h64, cudaStreamSynchronize(h64->stream));
+    if (outer_host) *outer_host = outer;
+    if (inner_total_host) *inner_total_host = inner_total;
+    if (relres_host) *relres_host = rel;
     return DWF_OK;
 }
 

@@ -60,6 +60,47 @@ __global__ void reorder_gauge_kernel(const R* __restrict__ canon, R* __restrict_
     native[gid * 2 + 1] = sign * canon[ci + 1];
 }
 
+// Precision conversion between the native layouts of two handles on the same lattice (mixed-precision solve).  The two
+// handles may order their sites differently (tile shape depends on the precision): inv_src[lexicographic site] = index of
+// that site in the source order of its parity, lex_dst[parity][site] = lexicographic site of the destination order.
+__global__ void invert_lex_kernel(const int* __restrict__ lex /*[2][V4h]*/, int* __restrict__ inv /*[V4]*/, long long V4h) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= 2 * V4h) return;
+    inv[lex[gid]] = (int)(gid % V4h);
+}
+// one thread per (destination block, component c, pair of s): handles s = 2j, 2j+1
+template <typename RS, typename RD>
+__global__ void convert_kernel(const typename Prec<RS>::G* __restrict__ src, typename Prec<RD>::G* __restrict__ dst,
+                               const int* __restrict__ inv_src, const int* __restrict__ lex_dst, long long V4h,
+                               int Ls, int nrhs, int sg_src, int sg_dst, int parities) {
+    const int KP = Ls / 2;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)parities * V4h * nrhs * 12 * KP;
+    if (gid >= total) return;
+    const int j = (int)(gid % KP);
+    const int c = (int)((gid / KP) % 12);
+    const int r = (int)((gid / (12 * KP)) % nrhs);
+    const long long ps = gid / ((long long)12 * KP * nrhs);           // p * V4h + destination site
+    const long long p = ps / V4h, sd = ps - p * V4h;
+    const long long ss = inv_src[lex_dst[ps]];
+    const size_t half_s = (size_t)V4h * nrhs * 12 * (Ls / Prec<RS>::VL), half_d = (size_t)V4h * nrhs * 12 * (Ls / Prec<RD>::VL);
+    const size_t bs = (size_t)blk_index(ss, r, nrhs, sg_src), bd = (size_t)blk_index(sd, r, nrhs, sg_dst);
+    double re0, im0, re1, im1;
+    if constexpr (Prec<RS>::VL == 2) {
+        const float4 g = src[p * half_s + (bs * 12 + c) * KP + j];
+        re0 = g.x; re1 = g.y; im0 = g.z; im1 = g.w;
+    } else {
+        const double2 g0 = src[p * half_s + (bs * 12 + c) * Ls + 2 * j], g1 = src[p * half_s + (bs * 12 + c) * Ls + 2 * j + 1];
+        re0 = g0.x; im0 = g0.y; re1 = g1.x; im1 = g1.y;
+    }
+    if constexpr (Prec<RD>::VL == 2) {
+        dst[p * half_d + (bd * 12 + c) * KP + j] = make_float4((float)re0, (float)re1, (float)im0, (float)im1);
+    } else {
+        dst[p * half_d + (bd * 12 + c) * Ls + 2 * j] = make_double2(re0, im0);
+        dst[p * half_d + (bd * 12 + c) * Ls + 2 * j + 1] = make_double2(re1, im1);
+    }
+}
+
 // Gathered links for the tiled stencil (dwf_tile.cuh): per site [mu][U_mu(x) 18 | U_mu(x-mu) 18] + padding,
 // pre-scaled by -1/2 (exact), so that a tile's links are one contiguous run and need no index lookup.
 template <typename R>

@@ -53,6 +53,10 @@ _SIGNATURES = {
                                           ctypes.POINTER(ctypes.c_double)]),
     "dwf_solve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_int,
                                  ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]),
+    "dwf_convert": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
+    "dwf_solve_mixed": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_double,
+                                       ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_int),
+                                       ctypes.POINTER(ctypes.c_double)]),
     "dwf_launch_count": (ctypes.c_longlong, [ctypes.c_void_p]),
     "dwf_last_error": (ctypes.c_char_p, [ctypes.c_void_p]),
 }
@@ -244,6 +248,20 @@ class Dwf:
         self._check(self.lib.dwf_solve(self._h, ctypes.c_void_p(eta.data_ptr()), ctypes.c_void_p(psi.data_ptr()), tol, max_iters,
                                        ctypes.byref(it), ctypes.byref(rr)))
         return int(it.value), float(rr.value)
+
+    def convert_to(self, dst: "Dwf", inp: torch.Tensor, nrhs: int, out: torch.Tensor = None) -> torch.Tensor:
+        """Native field of this handle -> native field of `dst` (other precision / site order)."""
+        if out is None:
+            out = dst.field(nrhs)
+        self._check(self.lib.dwf_convert(self._h, dst._h, ctypes.c_void_p(inp.data_ptr()), ctypes.c_void_p(out.data_ptr()), nrhs))
+        return out
+
+    def solve_mixed(self, h32: "Dwf", eta: torch.Tensor, psi: torch.Tensor, tol: float, inner_tol: float, max_outer: int, max_inner: int):
+        """self = the fp64 handle.  Returns (outer corrections, total fp32 CG iterations, final relative residual)."""
+        o, i, rr = ctypes.c_int(), ctypes.c_int(), ctypes.c_double()
+        self._check(self.lib.dwf_solve_mixed(self._h, h32._h, ctypes.c_void_p(eta.data_ptr()), ctypes.c_void_p(psi.data_ptr()), tol, inner_tol,
+                                             max_outer, max_inner, ctypes.byref(o), ctypes.byref(i), ctypes.byref(rr)))
+        return int(o.value), int(i.value), float(rr.value)
 
     def launch_count(self) -> int:
         return int(self.lib.dwf_launch_count(self._h))

@@ -289,3 +289,31 @@ def test_cg_multi_rhs(oracle, prec):
     x1 = rig.d.field(1, half=True, zero=True)
     h1 = rig.d.cg_schur(rig.native(b[0:1], 0), x1, iters)
     assert np.max(np.abs(np.array(h1) - hist[:, 0]) / hist[:, 0]) < (1e-12 if prec == "f64" else 1e-5)
+
+
+# ------------------------------------------------------------------ precision conversion + mixed-precision solve (rest of N3)
+def test_convert_and_mixed_precision_solve(oracle):
+    import torch
+    from paper_2103_05034_b200 import Dwf, DWF_F32
+    L, Ls, mass = (8, 4, 4, 8), 16, 0.05                               # fp64: 16-site tiles, fp32: 32-site tiles -> different site orders
+    r64 = Rig(L, Ls, "f64", mass, seed_U=91, ws_nrhs=1)
+    h32 = Dwf(L, Ls, M5, mass, DWF_F32)
+    h32.set_gauge(torch.from_numpy(np.ascontiguousarray(r64.U)).to(torch.complex64).cuda())
+    h32.set_workspace(1)
+    eta = r64.spinor(2, 92)
+    # conversion: fp64 native -> fp32 native -> canonical == canonical rounded to fp32 (bit exact), and back
+    n64 = r64.native(eta)
+    n32 = r64.d.convert_to(h32, n64, 2)
+    can32 = h32.export(n32, 2).cpu().numpy()
+    assert np.array_equal(can32, eta.astype(np.complex64))
+    back = h32.convert_to(r64.d, n32, 2)
+    assert np.array_equal(r64.canonical(back, 2), eta.astype(np.complex64).astype(np.complex128))
+    # mixed-precision solve to fp64 accuracy
+    e1 = r64.native(eta[0:1])
+    psi = r64.d.field(1)
+    outer, inner, relres = r64.d.solve_mixed(h32, e1, psi, 1e-11, 1e-4, 20, 2000)
+    got = r64.canonical(psi, 1)
+    assert 2 <= outer <= 8 and relres <= 1e-11
+    assert rel_l2(oracle.ddw(r64.U, got, M5, mass), eta[0:1]) < 3e-11   # the oracle's operator agrees with the residual
+    psi_or, _ = oracle.solve_rb(r64.U, eta[0:1], M5, mass, 1e-13, 4000)
+    assert rel_l2(got, psi_or) < 1e-9
