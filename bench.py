@@ -265,7 +265,7 @@ def run_only_config4(args, dev):
         out = {"only": "ddw_48", "ms": round(ms, 3), "GB/s": round(by / ms / 1e6, 1), "GFlop/s": round(FLOP_PER_SITE * v5 / ms / 1e6, 1),
                "frac_of_hbm_peak": round(by / ms / 1e6 / peaks()[0], 4)}
     else:
-        d.set_workspace(1)
+        d.set_workspace(1, half_fields=5)
         bb, xx = d.field(1, half=True).normal_(generator=g), d.field(1, half=True, zero=True)
         d.cg_schur(bb, xx, 3)
         xx.zero_(); torch.cuda.synchronize()

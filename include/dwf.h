@@ -70,9 +70,13 @@ int dwf_destroy(dwf_handle h);
 /* Stream on which all later work of this handle is enqueued (a cudaStream_t; NULL = default). */
 int dwf_set_stream(dwf_handle h, void* cuda_stream);
 
-/* Scratch for dwf_apply(SCHUR_EO), dwf_chebyshev(_subspace), dwf_power_lambda_max, dwf_cg_schur, dwf_apply_host with up to `nrhs`
- * right-hand sides.  The library never allocates field memory: the caller provides a device buffer
- * of at least dwf_workspace_bytes() bytes and keeps it alive while the handle uses it. */
+/* Scratch.  The library never allocates field memory: the caller provides a device buffer and keeps it alive while
+ * the handle uses it.  dwf_workspace_bytes(h, nrhs) is enough for EVERY call with up to nrhs right-hand sides
+ * (12 half fields + 256 bytes); a caller that makes only some calls may register less -- each call below states
+ * its need in half fields of nrhs right-hand sides (dwf_field_bytes(h, nrhs, 1)) and returns DWF_ENOWORKSPACE if
+ * the registered buffer is smaller: SCHUR_EO 1, SCHUR_EO_ALT 2, MPVDAG_M 2, dwf_chebyshev 4, dwf_chebyshev_subspace 6,
+ * dwf_chebyshev_smoother 8, dwf_power_lambda_max 4, dwf_cg_schur(_multi) 5, dwf_apply_host 5, dwf_solve 8,
+ * dwf_solve_mixed 6 (fp64 handle) + 12 (fp32 handle). */
 size_t dwf_workspace_bytes(dwf_handle h, int nrhs);
 int dwf_set_workspace(dwf_handle h, void* dev_ptr, size_t nbytes);
 

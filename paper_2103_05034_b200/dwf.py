@@ -139,9 +139,11 @@ class Dwf:
     def workspace_bytes(self, nrhs: int) -> int:
         return int(self.lib.dwf_workspace_bytes(self._h, nrhs))
 
-    def set_workspace(self, nrhs: int):
-        """Allocate (torch) and register a workspace big enough for `nrhs` right-hand sides."""
-        n = self.workspace_bytes(nrhs)
+    def set_workspace(self, nrhs: int, half_fields: int = None):
+        """Allocate (torch) and register a workspace for `nrhs` right-hand sides: big enough for every call of the library
+        (dwf_workspace_bytes), or for `half_fields` half fields when the caller knows which calls it makes (include/dwf.h
+        states each call's need; e.g. 5 for dwf_cg_schur at 48^3 x 96 x 24, where the full 12 would not fit beside the fields)."""
+        n = self.workspace_bytes(nrhs) if half_fields is None else self.field_bytes(nrhs, half=True) * half_fields + 256
         if self._ws is None or self._ws.numel() < n:
             self._ws = None
             self._ws = torch.empty(n, dtype=torch.uint8, device=self.device)

@@ -144,7 +144,7 @@ def test_config4_ddw_sampled_and_cg_invariants(oracle):
     del Ha, Hb, b2, psi
     # ---- 100 CG iterations on the even half: recursive residual == true residual, computed with
     # separately launched operator applications
-    d.set_workspace(1)
+    d.set_workspace(1, half_fields=5)                               # CG + Schur only: 5 x 12.2 GB
     hb = d.field_bytes(1, half=True) // 4
     b = x[:hb].clone()
     del x
