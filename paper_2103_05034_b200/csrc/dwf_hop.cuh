@@ -212,9 +212,10 @@ __device__ __forceinline__ void self_term(CV<double> (&res)[12], const double2* 
 // Gamma5 = gamma5 R5 (eq. 6, R6): lane group k of a block goes to group K-1-k (fp32: the two lanes
 // of the group also swap).
 //
-// Work decomposition: a CTA of 256 threads handles G = 256/K consecutive sites (one tile of the native
-// site order) for ONE right-hand side; thread = (site in tile, lane group k).  The 8 links of each of
-// the G sites are fetched once per CTA into shared memory and read back as 128-bit broadcasts.
+// Generic stencil kernel (any even lattice >= 4, any even Ls; the production path for lattices made of whole tiles is
+// hop_tile_kernel in dwf_tile.cuh).  A CTA of HOP_THREADS threads handles min(HOP_THREADS/8, HOP_THREADS/K) consecutive
+// sites for ONE right-hand side; thread = (site, lane group k).  The 8 links of each of the CTA's sites are fetched once
+// per CTA into shared memory and read back as 128-bit broadcasts; neighbour blocks come through L1 (LDG.NC).
 template <typename R, int LS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY>
 __global__ void __launch_bounds__(HOP_THREADS, 512 / HOP_THREADS)
 hop_kernel(const HopArgs<R> a) {
