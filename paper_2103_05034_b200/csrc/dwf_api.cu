@@ -248,8 +248,10 @@ static int reorder_spinor(dwf_ctx* h, const void* canon_in, void* canon_out, voi
     G* n0; G* n1; const int* l0; const int* l1; unsigned ny;
     if (parity < 0) { n0 = (G*)native; n1 = (G*)native + per_parity; l0 = h->lex; l1 = h->lex + h->V4h; ny = 2; }
     else            { n0 = n1 = (G*)native; l0 = l1 = h->lex + (size_t)parity * h->V4h; ny = 1; }
-    dim3 grid((unsigned)((per_parity + 255) / 256), ny);
-    reorder_spinor_kernel<R, IMPORT><<<grid, 256, 0, h->stream>>>((const R*)canon_in, (R*)canon_out, n0, n1, l0, l1, h->V4h, h->V4, h->Ls, nrhs, h->sg_shift);
+    const long long pairs = h->V4h * nrhs;                                       // one warp per (site, rhs) block
+    dim3 grid((unsigned)((pairs + 3) / 4), ny);
+    const size_t dsm = 4 * 24 * (size_t)h->Ls * sizeof(R);
+    reorder_spinor_kernel<R, IMPORT><<<grid, 128, dsm, h->stream>>>((const R*)canon_in, (R*)canon_out, n0, n1, l0, l1, h->V4h, h->V4, h->Ls, nrhs, h->sg_shift);
     LAUNCH_CHECK(h);
     return DWF_OK;
 }

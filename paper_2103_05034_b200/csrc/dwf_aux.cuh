@@ -8,37 +8,51 @@ namespace dwf {
 // ------------------------------------------------------------------------------------------------
 // a1. canonical <-> native reorder.  canonical spinor: complex<R> [nrhs][Ls][V4 lex][12];
 // native: group index ((blk_index(site, r)*12 + c)*K + k), K = Ls/VL, group k holds lanes s = k*VL .. k*VL+VL-1.
-// One thread per native group; blockIdx.y = parity slot.
 // ------------------------------------------------------------------------------------------------
+// One warp per (site, rhs) block, staged through shared memory: the canonical side moves in 96R-byte runs (the 12 complex
+// components of one (s, site)), the native side in whole 16-byte groups of the contiguous block -- full sectors both ways.
+// blockIdx.y = parity slot; dynamic shared memory = (warps per CTA) x 24 Ls reals.
 template <typename R, bool IMPORT>
-__global__ void reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restrict__ canon_out,
-                                      typename Prec<R>::G* native0, typename Prec<R>::G* native1,
-                                      const int* __restrict__ lex0, const int* __restrict__ lex1,
-                                      long long V4h, long long V4, int Ls, int nrhs, int sg_shift) {
+__global__ void __launch_bounds__(128)
+reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restrict__ canon_out,
+                      typename Prec<R>::G* native0, typename Prec<R>::G* native1,
+                      const int* __restrict__ lex0, const int* __restrict__ lex1,
+                      long long V4h, long long V4, int Ls, int nrhs, int sg_shift) {
     using G = typename Prec<R>::G;
     constexpr int VL = Prec<R>::VL;
-    const int K = Ls / VL;
-    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= V4h * 12 * nrhs * K) return;
-    // c fastest so that canonical accesses of neighbouring threads are contiguous (12 complex per site)
-    const int c = (int)(gid % 12);
-    const long long t2 = gid / 12;
-    const long long site = t2 % V4h;
-    const int lg = (int)(t2 / V4h);
-    G* native = blockIdx.y ? native1 : native0;
-    const int* lex = blockIdx.y ? lex1 : lex0;
-    const long long lx = lex[site];
-    const int r = lg / K, k = lg % K, s = k * VL;
-    const size_t nidx = ((size_t)blk_index(site, r, nrhs, sg_shift) * 12 + c) * K + k;
-    const size_t c0 = ((((size_t)r * Ls + s) * V4 + lx) * 12 + c) * 2;
-    const size_t sstride = (size_t)V4 * 12 * 2;          // to the next s
+    extern __shared__ __align__(16) unsigned char smem_reorder[];
+    const int K = Ls / VL, NG = 12 * K;                         // groups per block
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    R* buf = reinterpret_cast<R*>(smem_reorder) + (size_t)warp * 24 * Ls;
+    const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + warp;     // (site, rhs) pair of this parity
+    if (wid >= V4h * nrhs) return;                               // whole warps leave together
+    const long long site = wid / nrhs;
+    const int r = (int)(wid - site * nrhs);
+    G* native = (blockIdx.y ? native1 : native0) + (size_t)blk_index(site, r, nrhs, sg_shift) * NG;
+    const long long lx = (blockIdx.y ? lex1 : lex0)[site];
+    // position of the real (s, c, reim) inside the native block, in reals
+    auto npos = [&](int s, int c, int reim) -> int {
+        if constexpr (VL == 2) return ((c * K + (s >> 1)) << 2) + (reim << 1) + (s & 1);
+        else                   return ((c * K + s) << 1) + reim;
+    };
     if constexpr (IMPORT) {
-        if constexpr (VL == 2) native[nidx] = make_float4(canon_in[c0], canon_in[c0 + sstride], canon_in[c0 + 1], canon_in[c0 + sstride + 1]);
-        else                   native[nidx] = make_double2(canon_in[c0], canon_in[c0 + 1]);
+        for (int idx = lane; idx < Ls * 12; idx += 32) {         // idx = s*12 + c: one complex number per lane, 12 lanes per 96R-byte run
+            const int s = idx / 12, c = idx - s * 12;
+            const size_t ci = ((((size_t)r * Ls + s) * V4 + lx) * 12 + c) * 2;
+            buf[npos(s, c, 0)] = canon_in[ci]; buf[npos(s, c, 1)] = canon_in[ci + 1];
+        }
+        __syncwarp();
+        const G* bg = reinterpret_cast<const G*>(buf);
+        for (int g = lane; g < NG; g += 32) native[g] = bg[g];
     } else {
-        const G g = native[nidx];
-        if constexpr (VL == 2) { canon_out[c0] = g.x; canon_out[c0 + sstride] = g.y; canon_out[c0 + 1] = g.z; canon_out[c0 + sstride + 1] = g.w; }
-        else                   { canon_out[c0] = g.x; canon_out[c0 + 1] = g.y; }
+        G* bg = reinterpret_cast<G*>(buf);
+        for (int g = lane; g < NG; g += 32) bg[g] = native[g];
+        __syncwarp();
+        for (int idx = lane; idx < Ls * 12; idx += 32) {
+            const int s = idx / 12, c = idx - s * 12;
+            const size_t ci = ((((size_t)r * Ls + s) * V4 + lx) * 12 + c) * 2;
+            canon_out[ci] = buf[npos(s, c, 0)]; canon_out[ci + 1] = buf[npos(s, c, 1)];
+        }
     }
 }
 
