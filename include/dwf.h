@@ -75,7 +75,7 @@ int dwf_set_stream(dwf_handle h, void* cuda_stream);
  * (12 half fields + 256 bytes); a caller that makes only some calls may register less -- each call below states
  * its need in half fields of nrhs right-hand sides (dwf_field_bytes(h, nrhs, 1)) and returns DWF_ENOWORKSPACE if
  * the registered buffer is smaller: SCHUR_EO 1, SCHUR_EO_ALT 2, MPVDAG_M 2, dwf_chebyshev 4, dwf_chebyshev_subspace 6,
- * dwf_chebyshev_smoother 8, dwf_power_lambda_max 4, dwf_cg_schur(_multi) 5, dwf_apply_host 5, dwf_solve 8,
+ * dwf_chebyshev_smoother 8, dwf_power_lambda_max 4, dwf_cg_schur(_multi) 5, dwf_cg_normal 8, dwf_apply_host 5, dwf_solve 8,
  * dwf_solve_mixed 6 (fp64 handle) + 12 (fp32 handle). */
 size_t dwf_workspace_bytes(dwf_handle h, int nrhs);
 int dwf_set_workspace(dwf_handle h, void* dev_ptr, size_t nbytes);
@@ -146,6 +146,11 @@ int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, doub
  * of them).  b_even, x_even: even half fields of nrhs right-hand sides; resid2_hist_host (may be NULL): (iters+1) * nrhs
  * values, [k][r] = |r_k|^2 of rhs r.  Uses the workspace (5 half fields of nrhs right-hand sides). */
 int dwf_cg_schur_multi(dwf_handle h, const void* b_even, void* x_even, int iters, int nrhs, double* resid2_hist_host);
+
+/* Unpreconditioned CGNR (Table V, eq. 9): `iters` iterations of the same CG on M^dag M x = b with M = D_DW
+ * (M^dag M = H_DW^2, eq. 11), FULL native fields of nrhs right-hand sides, x holds x_0 on entry.  History as in
+ * dwf_cg_schur_multi.  Uses the workspace (8 half fields of nrhs right-hand sides). */
+int dwf_cg_normal(dwf_handle h, const void* b, void* x, int iters, int nrhs, double* resid2_hist_host);
 
 /* Complete red-black solve of D_DW psi = eta (Table V; eq. 9), nrhs = 1, full native fields:
  *   eta'_e = eta_e - M_eo M_oo^-1 eta_o;  CGNR on M_pc^dag M_pc psi_e = M_pc^dag eta'_e from psi_e = 0, stopped when

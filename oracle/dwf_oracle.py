@@ -201,6 +201,28 @@ def chebyshev_smoother(U, r, M5: float, mass: float, N: int, a: float, b: float)
     return out
 
 
+def cg_normal(U, b, M5: float, mass: float, iters: int, x0=None):
+    """Unpreconditioned CGNR (Table V L384, eq. 9 L73): Hestenes-Stiefel CG [29] on A = M^dag M, M = D_DW, with the true adjoint;
+    one right-hand side.  Returns (x_iters, [|r_k|^2 for k = 0..iters])."""
+    b = _c(b)
+    A = lambda v: ddw(U, ddw(U, v, M5, mass), M5, mass, dagger=True)
+    x = np.zeros_like(b) if x0 is None else _c(x0).copy()
+    r = b - A(x)
+    p = r.copy()
+    rr = float(np.vdot(r, r).real)
+    hist = [rr]
+    for _ in range(iters):
+        Ap = A(p)
+        alpha = rr / float(np.vdot(p, Ap).real)
+        x = x + alpha * p
+        r = r - alpha * Ap
+        rr_new = float(np.vdot(r, r).real)
+        p = r + (rr_new / rr) * p
+        rr = rr_new
+        hist.append(rr)
+    return x, np.array(hist)
+
+
 def _parity_mask(L, parity: int) -> np.ndarray:
     Lx, Ly, Lz, Lt = L
     t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")

@@ -750,24 +750,36 @@ extern "C" int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs
 // <p_k, A p_k> = |M p_k|^2 at scal[iters+1+k].
 // ------------------------------------------------------------------------------------------------
 template <typename R>
-static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, int nrhs = 1, double tol_rel = 0.0, int check_every = 10, int* done = nullptr) {
+// kind 0: A = M_pc^dag M_pc on even half fields (red-black CGNR);  kind 1: A = M^dag M = H_DW^2 on full fields (unpreconditioned
+// CGNR, Table V).  In both A p = O2(O1 p) with <p, A p> = |O1 p|^2.
+static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, int nrhs = 1, double tol_rel = 0.0, int check_every = 10, int* done = nullptr,
+                int kind = 0) {
     using G = typename Prec<R>::G;
-    const size_t hb = half_bytes(h, nrhs);
-    const long long ng = half_groups(h, nrhs);
+    const size_t hb = half_bytes(h, nrhs) * (kind ? 2 : 1);
+    const long long ng = half_groups(h, nrhs) * (kind ? 2 : 1);
+    auto op1 = [&](const void* in, void* out, void* tmp, double* norm_out) -> int {
+        if (kind == 0) return schur_op(h, false, in, out, tmp, nrhs, norm_out);
+        if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, in, out, nrhs)) return rc;
+        return norm_out ? reduce_to(h, true, out, nullptr, nrhs, 0, norm_out, 1, 1) : DWF_OK;
+    };
+    auto op2 = [&](const void* in, void* out, void* tmp) -> int {
+        if (kind == 0) return schur_op(h, true, in, out, tmp, nrhs);
+        return full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, in, out, nrhs);
+    };
     const int BS = run_groups(h);
     G* r = (G*)h->ws; G* p = (G*)((char*)h->ws + hb); G* w = (G*)((char*)h->ws + 2 * hb);
     G* q = (G*)((char*)h->ws + 3 * hb); void* tmp = (char*)h->ws + 4 * hb;
     double* hist = h->scal; double* pAp = h->scal + (size_t)(iters + 1) * nrhs;     // hist[k*nrhs + r], pAp[k*nrhs + r]
     const unsigned blocks = blas_blocks(h, ng, (long long)BS * nrhs);
     cudaStream_t st = h->stream;
-    if (int rc = schur_op(h, false, x, w, tmp, nrhs)) return rc;
-    if (int rc = schur_op(h, true, w, q, tmp, nrhs)) return rc;
+    if (int rc = op1(x, w, tmp, nullptr)) return rc;
+    if (int rc = op2(w, q, tmp)) return rc;
     cg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, q, r, p, ng, BS, nrhs, h->partial); LAUNCH_CHECK(h);
     reduce_final_kernel<<<nrhs, 256, 0, st>>>(h->partial, (int)blocks, nrhs, hist, 1, 1); LAUNCH_CHECK(h);
     for (int k = 0; k < iters; k++) {
         double* hk = hist + (size_t)k * nrhs; double* hk1 = hk + nrhs; double* pk = pAp + (size_t)k * nrhs;
-        if (int rc = schur_op(h, false, p, w, tmp, nrhs, pk)) return rc;           // w = M p and <p, A p> = |w|^2
-        if (int rc = schur_op(h, true, w, q, tmp, nrhs)) return rc;
+        if (int rc = op1(p, w, tmp, pk)) return rc;                                // w = O1 p and <p, A p> = |w|^2
+        if (int rc = op2(w, q, tmp)) return rc;
         cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, BS, nrhs, hk, pk, h->partial); LAUNCH_CHECK(h);
         reduce_final_kernel<<<nrhs, 256, 0, st>>>(h->partial, (int)blocks, nrhs, hk1, 1, 1); LAUNCH_CHECK(h);
         cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, BS, nrhs, hk1, hk); LAUNCH_CHECK(h);
@@ -782,7 +794,7 @@ static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, int nrhs = 1, dou
     return DWF_OK;
 }
 
-static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int iters, int nrhs, double* hist_host) {
+static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int iters, int nrhs, double* hist_host, int kind = 0) {
     if (!h) return DWF_EINVAL;
     if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
     if (iters < 0 || 2 * (long long)(iters + 1) * nrhs > SCAL_DOUBLES) FAIL(h, DWF_EINVAL, "iters out of range");
@@ -790,7 +802,7 @@ static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int ite
     if (int rc = check_field(h, x_even, "x_even")) return rc;
     if (b_even == x_even) FAIL(h, DWF_EINVAL, "b == x");
     if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
-    if (int rc = need_ws(h, 5 * half_bytes(h, nrhs))) return rc;
+    if (int rc = need_ws(h, (kind ? 8 : 5) * half_bytes(h, nrhs))) return rc;
     // The host loop only enqueues (alpha, beta live on the device).  DWF_CG_GRAPH=1 captures the whole solve into a
     // CUDA graph and launches it as one unit; measured on B200 (8^4x16: 7037 vs 7388 it/s, 16^3x32x16: no change)
     // the plain stream launches are already back to back, so the graph is off by default.
@@ -802,7 +814,7 @@ static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int ite
         cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
         CUDA_TRY(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
         h->stream = h->cap_stream;
-        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs) : cg_t<double>(h, b_even, x_even, iters, nrhs);
+        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind) : cg_t<double>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind);
         h->stream = user;
         cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
         if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -814,7 +826,7 @@ static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int ite
         cudaGraphDestroy(graph);
         if (e != cudaSuccess) FAIL(h, DWF_ECUDA, "CUDA graph of the CG loop: %s", cudaGetErrorString(e));
     } else {
-        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs) : cg_t<double>(h, b_even, x_even, iters, nrhs);
+        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind) : cg_t<double>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind);
         if (rc) return rc;
     }
     const size_t nh = (size_t)(iters + 1) * nrhs;
@@ -829,6 +841,9 @@ extern "C" int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int 
 }
 extern "C" int dwf_cg_schur_multi(dwf_handle h, const void* b_even, void* x_even, int iters, int nrhs, double* hist_host) {
     return cg_schur_impl(h, b_even, x_even, iters, nrhs, hist_host);
+}
+extern "C" int dwf_cg_normal(dwf_handle h, const void* b, void* x, int iters, int nrhs, double* hist_host) {
+    return cg_schur_impl(h, b, x, iters, nrhs, hist_host, 1);
 }
 
 // ------------------------------------------------------------------------------------------------

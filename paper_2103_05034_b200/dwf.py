@@ -51,6 +51,8 @@ _SIGNATURES = {
                                     ctypes.POINTER(ctypes.c_double)]),
     "dwf_cg_schur_multi": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
                                           ctypes.POINTER(ctypes.c_double)]),
+    "dwf_cg_normal": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
+                                     ctypes.POINTER(ctypes.c_double)]),
     "dwf_solve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_int,
                                  ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]),
     "dwf_convert": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
@@ -242,6 +244,11 @@ class Dwf:
         """Returns the history as a list of (iters+1) lists of nrhs values."""
         hist = (ctypes.c_double * ((iters + 1) * nrhs))()
         self._check(self.lib.dwf_cg_schur_multi(self._h, ctypes.c_void_p(b_even.data_ptr()), ctypes.c_void_p(x_even.data_ptr()), iters, nrhs, hist))
+        return [[float(hist[k * nrhs + r]) for r in range(nrhs)] for k in range(iters + 1)]
+
+    def cg_normal(self, b: torch.Tensor, x: torch.Tensor, iters: int, nrhs: int):
+        hist = (ctypes.c_double * ((iters + 1) * nrhs))()
+        self._check(self.lib.dwf_cg_normal(self._h, ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), iters, nrhs, hist))
         return [[float(hist[k * nrhs + r]) for r in range(nrhs)] for k in range(iters + 1)]
 
     def solve(self, eta: torch.Tensor, psi: torch.Tensor, tol: float, max_iters: int):

@@ -317,3 +317,20 @@ def test_convert_and_mixed_precision_solve(oracle):
     assert rel_l2(oracle.ddw(r64.U, got, M5, mass), eta[0:1]) < 3e-11   # the oracle's operator agrees with the residual
     psi_or, _ = oracle.solve_rb(r64.U, eta[0:1], M5, mass, 1e-13, 4000)
     assert rel_l2(got, psi_or) < 1e-9
+
+
+# ------------------------------------------------------------------ unpreconditioned CGNR on M^dag M (Table V)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_cg_normal(oracle, prec):
+    L, Ls, mass, nrhs, iters = (4, 4, 4, 8), 16, 0.05, 2, 25
+    rig = Rig(L, Ls, prec, mass, seed_U=95, ws_nrhs=nrhs)
+    b = rig.spinor(nrhs, 96)
+    bn = rig.native(b)
+    xn = rig.d.field(nrhs, zero=True)
+    hist = np.array(rig.d.cg_normal(bn, xn, iters, nrhs))
+    x = rig.canonical(xn, nrhs)
+    tol_h, tol_x = (1e-9, 1e-10) if prec == "f64" else (1e-4, 1e-5)
+    for r in range(nrhs):
+        x_or, h_or = oracle.cg_normal(rig.U, b[r:r + 1], M5, mass, iters)
+        assert np.max(np.abs(hist[:, r] - h_or) / h_or) < tol_h, r
+        assert rel_l2(x[r:r + 1], x_or) < tol_x, r

@@ -290,3 +290,22 @@ def test_mpc_alt_against_dense(oracle):
     mpc = oracle.mpc(U, x, M5, MASS)
     assert rel(oracle.mpp_inv(mpc, M5, MASS, 0)[0].reshape(-1)[e], A @ xe) < 1e-12
 
+
+# ---------------------------------------------------------------- unpreconditioned CGNR (Table V)
+def test_cg_normal_against_dense(oracle):
+    L, Ls = (4, 2, 2, 2), 4
+    U = gen.gauge_random(L, 5)
+    b = gen.spinor_gaussian(L, Ls, 1, 14)
+    D = dense.ddw_5d(U, L, Ls, M5, MASS)
+    A = D.conj().T @ D
+    want = np.linalg.solve(A, b[0].reshape(-1))
+    x, hist = oracle.cg_normal(U, b, M5, MASS, 300)
+    assert rel(x[0].reshape(-1), want) < 1e-8 and hist[-1] < 1e-16 * hist[0]
+    # true residual = recursive residual; A-norm of the error decreases monotonically (textbook CG)
+    xs = [oracle.cg_normal(U, b, M5, MASS, k)[0][0].reshape(-1) for k in (5, 10, 20, 40)]
+    errs = [np.vdot(v - want, A @ (v - want)).real for v in xs]
+    assert all(e2 < e1 for e1, e2 in zip(errs, errs[1:]))
+    x20, h20 = oracle.cg_normal(U, b, M5, MASS, 20)
+    rtrue = b[0].reshape(-1) - A @ x20[0].reshape(-1)
+    assert abs(np.vdot(rtrue, rtrue).real - h20[-1]) / h20[-1] < 1e-9
+
