@@ -188,6 +188,32 @@ def run_only(args, dev):
                           "H_applies": applies, "us_per_apply": round(1e3 * ms / applies, 1), "vectors/s": round(nvec / ms * 1e3, 1),
                           "GFlop/s": round(FLOP_PER_SITE * V5 * applies / ms / 1e6, 1)}), flush=True)
         return
+    if name == "solve":                                      # complete red-black solve of D_DW psi = eta to 1e-8 (fp32 + mixed)
+        d = Dwf(L, LS, M5, MASS, DWF_F32, device=dev)
+        U = gen.gauge_random(L, 1002)
+        d.set_gauge(torch.from_numpy(U).to(d.cdtype).to(dev))
+        d.set_workspace(1)
+        g = torch.Generator(device=dev); g.manual_seed(2011)
+        eta = d.field(1).normal_(generator=g); psi = d.field(1)
+        d.solve(eta, psi, 1e-5, 4000)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        iters, relres = d.solve(eta, psi, 1e-5, 4000)
+        torch.cuda.synchronize(); ms32 = (time.perf_counter() - t0) * 1e3
+        d64 = Dwf(L, LS, M5, MASS, DWF_F64, device=dev)
+        d64.set_gauge(torch.from_numpy(U).to(d64.cdtype).to(dev))
+        d64.set_workspace(1)
+        eta64 = d.convert_to(d64, eta, 1); psi64 = d64.field(1)
+        d64.solve_mixed(d, eta64, psi64, 1e-10, 1e-4, 20, 4000)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        outer, inner, rr = d64.solve_mixed(d, eta64, psi64, 1e-10, 1e-4, 20, 4000)
+        torch.cuda.synchronize(); msmx = (time.perf_counter() - t0) * 1e3
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        it64, rr64 = d64.solve(eta64, psi64, 1e-10, 4000)
+        torch.cuda.synchronize(); ms64 = (time.perf_counter() - t0) * 1e3
+        print(json.dumps({"only": name, "fp32_tol1e-5": {"iters": iters, "relres": relres, "ms": round(ms32, 2)},
+                          "mixed_tol1e-10": {"outer": outer, "inner_iters": inner, "relres": rr, "ms": round(msmx, 2)},
+                          "fp64_tol1e-10": {"iters": it64, "relres": rr64, "ms": round(ms64, 2)}}), flush=True)
+        return
     if name == "cg_8":                                       # BASELINE.json configs[1]: 8^4 x 16, 50 rb-CG iterations (launch-bound size)
         L8 = (8, 8, 8, 8)
         d = Dwf(L8, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)
