@@ -57,7 +57,8 @@ enum { DWF_DHOP = 0, DWF_DDW = 1, DWF_HDW = 2, DWF_DPV = 3, DWF_SCHUR_EO = 4, DW
        DWF_DAGGER = 0x100 };
 
 enum { DWF_OK = 0, DWF_EINVAL = -1, DWF_ENOGAUGE = -2, DWF_ENOMEM = -3, DWF_ECUDA = -4,
-       DWF_EUNSUPPORTED = -5, DWF_ENOWORKSPACE = -6 };
+       DWF_EUNSUPPORTED = -5, DWF_ENOWORKSPACE = -6,
+       DWF_ERANGE = -7 /* a result left the range of the field's precision (dwf_chebyshev_subspace) */ };
 
 /* Create a handle.  L = {Lx,Ly,Lz,Lt}, each even and >= 4; Ls even, 2 <= Ls <= 64 (closed-form M_oo^{-1}
  * is instantiated for Ls in {4,8,12,16,24,32}: other Ls -> DWF_EUNSUPPORTED from SCHUR_EO/MOOINV/CG).
@@ -75,7 +76,8 @@ int dwf_set_stream(dwf_handle h, void* cuda_stream);
  * (12 half fields + 256 bytes); a caller that makes only some calls may register less -- each call below states
  * its need in half fields of nrhs right-hand sides (dwf_field_bytes(h, nrhs, 1)) and returns DWF_ENOWORKSPACE if
  * the registered buffer is smaller: SCHUR_EO 1, SCHUR_EO_ALT 2, MPVDAG_M 2, dwf_chebyshev 4, dwf_chebyshev_subspace 6,
- * dwf_chebyshev_smoother 8, dwf_power_lambda_max 4, dwf_cg_schur(_multi) 5, dwf_cg_normal 8, dwf_apply_host 5, dwf_solve 8,
+ * dwf_chebyshev_smoother 8, dwf_power_lambda_max 4, dwf_cg_schur(_multi) 5, dwf_cg_normal 8, dwf_bicgstab_pv 12, dwf_apply_host 4 + the
+ * operator's own need, dwf_solve 8,
  * dwf_solve_mixed 6 (fp64 handle) + 12 (fp32 handle). */
 size_t dwf_workspace_bytes(dwf_handle h, int nrhs);
 int dwf_set_workspace(dwf_handle h, void* dev_ptr, size_t nbytes);
@@ -96,9 +98,10 @@ int dwf_export(dwf_handle h, const void* native_dev, void* canonical_dev, int nr
 /* out = OP in, native layout, nrhs fields at once (1 <= nrhs <= 64); in != out. */
 int dwf_apply(dwf_handle h, int op, const void* in, void* out, int nrhs);
 
-/* Same operator, end to end from HOST canonical arrays: H2D copy, import, apply, export, D2H copy
- * (uses the workspace; synchronises).  For SCHUR_EO/MEE/MOOINV the arrays are full-lattice canonical
- * arrays of which only the even sites are read and written. */
+/* Same operator (every op of dwf_apply, DWF_DAGGER included), end to end from HOST canonical arrays: H2D copy, import,
+ * apply, export, D2H copy (synchronises).  Workspace: 4 half fields of staging + the operator's own need.  For the
+ * half-field ops SCHUR_EO/SCHUR_EO_ALT/MEE/MOOINV the arrays are full-lattice canonical arrays of which only the even
+ * sites are read; the odd sites of out_host are written as zero. */
 int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* out_host, int nrhs);
 
 /* out = T_order(2 (H_DW^2 - lo) / (hi - lo) - 1) in   (eq. 23, eq. 34; R10, R13, R14).
@@ -111,7 +114,9 @@ int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, const void* in,
  * All phi_k come from ONE three-term recurrence started at v ("all for the cost of the highest order", L229):
  * 2 m + 2 (nvec-1) delta operator applies.  phi = nvec consecutive full native fields of nrhs right-hand sides
  * each (phi_k at byte offset k * dwf_field_bytes(h, nrhs, 0)); eta != phi; m >= 0, delta >= 1, nvec >= 1,
- * 0 <= lambda_lo < lambda_max.  No normalisation (R14).  Uses the workspace (3 full fields). */
+ * 0 <= lambda_lo < lambda_max.  No normalisation (R14): outside [lambda_lo, lambda_max] T_m grows as cosh(m acosh|x|),
+ * so |phi_0|^2 and |phi_{nvec-1}|^2 are checked and DWF_ERANGE is returned when the precision of the handle overflowed
+ * (use an fp64 handle for m, lambda_lo with larger growth).  Uses the workspace (3 full fields).  Synchronises. */
 int dwf_chebyshev_subspace(dwf_handle h, int m, double lambda_lo, double lambda_max, int delta, int nvec,
                            const void* eta, void* phi, int nrhs);
 
@@ -151,6 +156,13 @@ int dwf_cg_schur_multi(dwf_handle h, const void* b_even, void* x_even, int iters
  * (M^dag M = H_DW^2, eq. 11), FULL native fields of nrhs right-hand sides, x holds x_0 on entry.  History as in
  * dwf_cg_schur_multi.  Uses the workspace (8 half fields of nrhs right-hand sides). */
 int dwf_cg_normal(dwf_handle h, const void* b, void* x, int iters, int nrhs, double* resid2_hist_host);
+
+/* BiCGSTAB (van der Vorst, PAPER.md ref. [31]) on the Pauli-Villars preconditioned system D_PV^dag D_DW x = b (PAPER.md
+ * L101-107; Table V), `iters` iterations, FULL native fields, nrhs = 1; x holds x_0 on entry and x_iters on return.
+ * resid2_hist_host (may be NULL) receives iters+1 values |r_i|^2 of the recursive residual r_i of this system.
+ * Complex <a,b> = sum conj(a) b; a vanishing denominator (zero right-hand side) freezes the iteration instead of dividing.
+ * Uses the workspace (12 half fields).  Enqueue-only (all scalars stay on the device); synchronises at the end. */
+int dwf_bicgstab_pv(dwf_handle h, const void* b, void* x, int iters, double* resid2_hist_host);
 
 /* Complete red-black solve of D_DW psi = eta (Table V; eq. 9), nrhs = 1, full native fields:
  *   eta'_e = eta_e - M_eo M_oo^-1 eta_o;  CGNR on M_pc^dag M_pc psi_e = M_pc^dag eta'_e from psi_e = 0, stopped when

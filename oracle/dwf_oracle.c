@@ -560,3 +560,112 @@ void oracle_ddw_sites(const int* L, int Ls, double M5, double mass, int64_t n, c
         }
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Site-list mode for the Schur operator (Table V): evaluate
+ *   M_pc psi_e = M_ee psi_e - M_eo M_oo^{-1} M_oe psi_e      (M_eo = M_oe = -1/2 D_hop, R8/R9)
+ * at a list of EVEN 4D sites x from gathered neighbourhoods: the 8 odd neighbours y_d of x and,
+ * for each of them, its 8 even neighbours z_{d,e} (the 33 even sites at taxicab distance 0 or 2,
+ * passed with repetition so that the loops below stay the plain definition).
+ * Direction slots: d, e = 2*mu (+mu) or 2*mu+1 (-mu).
+ *   coords[n][4]           (x,y,z,t) of x
+ *   self[n][Ls][12]        psi_e(x)
+ *   nbr2[n][8][8][Ls][12]  psi_e(z_{d,e}),  y_d = x + d,  z_{d,e} = y_d + e
+ *   links1[n][8][9]        slot 2*mu = U_mu(x),   2*mu+1 = U_mu(x - mu)        (as stored, undaggered)
+ *   links2[n][8][8][9]     [d] slot 2*nu = U_nu(y_d), 2*nu+1 = U_nu(y_d - nu)
+ *   out[n][Ls][12]
+ * M_oo^{-1}: generic elimination of the dense Ls x Ls s-matrix (dense_inverse), as in mpp_inv_core.
+ * dagger: M_pc^dag = M_ee^dag - M_oe^dag (M_oo^dag)^{-1} M_eo^dag with every factor a true adjoint:
+ * the block B(row, col) of the FORWARD operator is built from its definition and applied as B^dag
+ * from row to col (block_apply_dag), exactly as dhop_core does on full arrays.
+ * ------------------------------------------------------------------------------------------ */
+static void sites_block(const int* L, const int c_row[4], int mu, int dir, const cplx* u_fwd /* U_mu(row) */,
+                        const cplx* u_bwd /* U_mu(row - mu) */, hop_block_t* b) {
+    b->col = 0; b->sign = 1.0;
+    const int nc = c_row[mu] + dir;
+    if ((nc >= L[mu] || nc < 0) && mu == 3) b->sign = -1.0;
+    for (int a = 0; a < 4; a++) for (int bb = 0; bb < 4; bb++)
+        b->G[a][bb] = ((a == bb) ? 1.0 : 0.0) - (double)dir * GAMMA[mu][a][bb];
+    for (int a = 0; a < 3; a++) for (int bb = 0; bb < 3; bb++)
+        b->W[a][bb] = (dir > 0) ? u_fwd[a * 3 + bb] : conj(u_bwd[bb * 3 + a]);
+}
+
+int oracle_mpc_sites(const int* L, int Ls, double M5, double mass, int64_t n, const int* coords,
+                     const double* self_, const double* nbr2_, const double* links1_, const double* links2_,
+                     double* out_, int dagger) {
+    const cplx* self = (const cplx*)self_; const cplx* nbr2 = (const cplx*)nbr2_;
+    const cplx* links1 = (const cplx*)links1_; const cplx* links2 = (const cplx*)links2_; cplx* out = (cplx*)out_;
+    double* A = (double*)malloc(sizeof(double) * (size_t)Ls * Ls);
+    double* Ainv = (double*)malloc(sizeof(double) * (size_t)4 * Ls * Ls);
+    for (int sp = 0; sp < 4; sp++) {
+        mpp_dense(Ls, M5, mass, sp, A);
+        if (dagger) for (int i = 0; i < Ls; i++) for (int j = i + 1; j < Ls; j++) { double t = A[i * Ls + j]; A[i * Ls + j] = A[j * Ls + i]; A[j * Ls + i] = t; }
+        if (dense_inverse(Ls, A, Ainv + (size_t)sp * Ls * Ls)) { free(A); free(Ainv); return -1; }
+    }
+    #pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; i++) {
+        const int* cx = coords + 4 * i;
+        cplx* acc = (cplx*)calloc((size_t)Ls * 12, sizeof(cplx));      /* D_hop-type sum over the odd neighbours, row x */
+        cplx* ty = (cplx*)malloc(sizeof(cplx) * (size_t)Ls * 12);
+        cplx* vy = (cplx*)malloc(sizeof(cplx) * (size_t)Ls * 12);
+        for (int d = 0; d < 8; d++) {
+            const int mu = d / 2, dir = (d % 2 == 0) ? +1 : -1;
+            int cy[4] = {cx[0], cx[1], cx[2], cx[3]};
+            cy[mu] = (cx[mu] + dir + L[mu]) % L[mu];
+            /* ty = M_oe psi (or M_eo^dag psi) at the odd site y_d */
+            for (int k = 0; k < Ls * 12; k++) ty[k] = 0;
+            for (int e = 0; e < 8; e++) {
+                const int nu = e / 2, dire = (e % 2 == 0) ? +1 : -1;
+                const cplx* l2 = links2 + ((i * 8 + d) * 8) * 9;
+                const cplx* uy = l2 + (2 * nu) * 9;                 /* U_nu(y)      */
+                const cplx* uym = l2 + (2 * nu + 1) * 9;            /* U_nu(y - nu) */
+                const cplx* psi_z = nbr2 + (((i * 8 + d) * 8 + e) * (int64_t)Ls) * 12;
+                hop_block_t b;
+                if (!dagger) {
+                    sites_block(L, cy, nu, dire, uy, uym, &b);      /* B(row y, col z = y + e) */
+                    for (int s = 0; s < Ls; s++) block_apply(&b, psi_z + s * 12, ty + s * 12);
+                } else {
+                    /* B(row z, col y) of the forward operator: from z the site y lies in direction (nu, -dire);
+                     * U_nu(z) = U_nu(y - nu) when z = y - nu, U_nu(z - nu) = U_nu(y) when z = y + nu */
+                    int cz[4] = {cy[0], cy[1], cy[2], cy[3]};
+                    cz[nu] = (cy[nu] + dire + L[nu]) % L[nu];
+                    sites_block(L, cz, nu, -dire, uym, uy, &b);
+                    for (int s = 0; s < Ls; s++) block_apply_dag(&b, psi_z + s * 12, ty + s * 12);
+                }
+            }
+            for (int k = 0; k < Ls * 12; k++) ty[k] *= -0.5;
+            /* vy = M_oo^{-1} ty  (or (M_oo^dag)^{-1}) */
+            for (int s = 0; s < Ls; s++) for (int sp = 0; sp < 4; sp++) for (int c = 0; c < 3; c++) {
+                cplx a = 0;
+                for (int s2 = 0; s2 < Ls; s2++) a += Ainv[((size_t)sp * Ls + s) * Ls + s2] * ty[s2 * 12 + sp * 3 + c];
+                vy[s * 12 + sp * 3 + c] = a;
+            }
+            /* row x of D_hop_eo (or of D_hop_oe^dag) applied to vy */
+            const cplx* ux = links1 + (i * 8 + 2 * mu) * 9;         /* U_mu(x)      */
+            const cplx* uxm = links1 + (i * 8 + 2 * mu + 1) * 9;    /* U_mu(x - mu) */
+            hop_block_t b;
+            if (!dagger) {
+                sites_block(L, cx, mu, dir, ux, uxm, &b);           /* B(row x, col y_d) */
+                for (int s = 0; s < Ls; s++) block_apply(&b, vy + s * 12, acc + s * 12);
+            } else {
+                sites_block(L, cy, mu, -dir, uxm, ux, &b);          /* B(row y_d, col x): U_mu(y) = U_mu(x - mu) when y = x - mu, U_mu(y - mu) = U_mu(x) when y = x + mu */
+                for (int s = 0; s < Ls; s++) block_apply_dag(&b, vy + s * 12, acc + s * 12);
+            }
+        }
+        /* out = M_ee psi(x) - (-1/2) acc ;  M_ee = (5 - M5) + S  (adjoint: S transposed, scatter form) */
+        const cplx* sx = self + (i * (int64_t)Ls) * 12;
+        cplx* o = out + (i * (int64_t)Ls) * 12;
+        for (int k = 0; k < Ls * 12; k++) o[k] = (5.0 - M5) * sx[k] + 0.5 * acc[k];
+        for (int s = 0; s < Ls; s++) {
+            sblock_t blk[4];
+            const int nb = s_row_blocks(Ls, mass, s, blk);
+            for (int j = 0; j < nb; j++) for (int sp = 0; sp < 4; sp++) for (int c = 0; c < 3; c++) {
+                if (!dagger) o[s * 12 + sp * 3 + c] += blk[j].coef * blk[j].P[sp] * sx[blk[j].col * 12 + sp * 3 + c];
+                else         o[blk[j].col * 12 + sp * 3 + c] += blk[j].coef * blk[j].P[sp] * sx[s * 12 + sp * 3 + c];
+            }
+        }
+        free(acc); free(ty); free(vy);
+    }
+    free(A); free(Ainv);
+    return 0;
+}

@@ -223,17 +223,49 @@ def cg_normal(U, b, M5: float, mass: float, iters: int, x0=None):
     return x, np.array(hist)
 
 
+def bicgstab_pv(U, b, M5: float, mass: float, iters: int, x0=None):
+    """BiCGSTAB (van der Vorst, PAPER.md ref. [31] L671; the paper does not restate it, L120) on the Pauli-Villars preconditioned
+    system A x = b, A = M_PV^dag M = D_PV^dag D_DW (L101-107; Table V), one right-hand side, written out step by step in the
+    notation of the original algorithm (unpreconditioned form, rhat_0 = r_0, <a,b> = sum conj(a) b):
+        rho_i = <rhat0, r_{i-1}>;  beta = (rho_i/rho_{i-1})(alpha/omega_{i-1});  p_i = r_{i-1} + beta (p_{i-1} - omega_{i-1} v_{i-1});
+        v_i = A p_i;  alpha = rho_i/<rhat0, v_i>;  s = r_{i-1} - alpha v_i;  t = A s;  omega_i = <t,s>/<t,t>;
+        x_i = x_{i-1} + alpha p_i + omega_i s;  r_i = s - omega_i t.
+    Returns (x_iters, [|r_i|^2 for i = 0..iters])."""
+    b = _c(b)
+    A = lambda f: mpvdag_m(U, f, M5, mass)
+    x = np.zeros_like(b) if x0 is None else _c(x0).copy()
+    r = b - A(x)
+    rhat = r.copy()
+    rho_old = alpha = omega = 1.0 + 0.0j
+    v = np.zeros_like(b); p = np.zeros_like(b)
+    hist = [float(np.vdot(r, r).real)]
+    for _ in range(iters):
+        rho = np.vdot(rhat, r)
+        beta = (rho / rho_old) * (alpha / omega)
+        p = r + beta * (p - omega * v)
+        v = A(p)
+        alpha = rho / np.vdot(rhat, v)
+        s = r - alpha * v
+        t = A(s)
+        omega = np.vdot(t, s) / np.vdot(t, t)
+        x = x + alpha * p + omega * s
+        r = s - omega * t
+        rho_old = rho
+        hist.append(float(np.vdot(r, r).real))
+    return x, np.array(hist)
+
+
 def _parity_mask(L, parity: int) -> np.ndarray:
     Lx, Ly, Lz, Lt = L
     t, z, y, x = np.meshgrid(np.arange(Lt), np.arange(Lz), np.arange(Ly), np.arange(Lx), indexing="ij")
     return (((x + y + z + t) & 1) == parity)[None, None, :, :, :, :, None, None]
 
 
-def solve_rb(U, eta, M5: float, mass: float, tol: float, max_iters: int, check_every: int = 10):
+def solve_rb(U, eta, M5: float, mass: float, tol: float, max_iters: int):
     """D_DW psi = eta by the complete red-black solve (Table V, eq. 9), nrhs = 1:
-    eta'_e = eta_e - M_eo M_oo^-1 eta_o; CGNR on M_pc^dag M_pc psi_e = M_pc^dag eta'_e from 0, stopped at the first
-    multiple of `check_every` iterations with |r_k| <= tol |r_0| (or max_iters); psi_o = M_oo^-1 (eta_o - M_oe psi_e);
-    M_eo = M_oe = -1/2 Dhop (eq. 4-5).  Returns (psi, iterations)."""
+    eta'_e = eta_e - M_eo M_oo^-1 eta_o; CGNR on M_pc^dag M_pc psi_e = M_pc^dag eta'_e from 0, stopped at the FIRST iteration
+    k with |r_k| <= tol |r_0| (the textbook rule, tested every iteration; DESIGN.md reading R25) or at max_iters;
+    psi_o = M_oo^-1 (eta_o - M_oe psi_e); M_eo = M_oe = -1/2 Dhop (eq. 4-5).  Returns (psi, iterations)."""
     eta = _c(eta); L, Ls, _ = _geom(eta)
     me, mo = _parity_mask(L, 0), _parity_mask(L, 1)
     eta_e, eta_o = eta * me, eta * mo
@@ -243,7 +275,7 @@ def solve_rb(U, eta, M5: float, mass: float, tol: float, max_iters: int, check_e
     b = mpc(U, src, M5, mass, dagger=True)
     _, hist = cg_schur(U, b, M5, mass, max_iters)
     iters = max_iters
-    for k in range(check_every, max_iters + 1, check_every):
+    for k in range(1, max_iters + 1):
         if hist[k] <= tol * tol * hist[0]:
             iters = k
             break
@@ -308,4 +340,20 @@ def ddw_sites(L, Ls: int, M5: float, mass: float, coords, nbr, links) -> np.ndar
     out = np.empty((n, Ls, 4, 3), dtype=np.complex128)
     lib().oracle_ddw_sites(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass),
                            ctypes.c_int64(n), _p(coords), _p(nbr), _p(links), _p(out))
+    return out
+
+
+def mpc_sites(L, Ls: int, M5: float, mass: float, coords, self_, nbr2, links1, links2, dagger: bool = False) -> np.ndarray:
+    """Site-list mode: rows of M_pc (Table V) at sampled EVEN 4D sites from gathered neighbourhoods (see .c header)."""
+    coords = np.ascontiguousarray(coords, dtype=np.int32)
+    n = coords.shape[0]
+    self_ = _c(self_); nbr2 = _c(nbr2); links1 = _c(links1); links2 = _c(links2)
+    assert self_.shape == (n, Ls, 4, 3) and nbr2.shape == (n, 8, 8, Ls, 4, 3)
+    assert links1.shape == (n, 8, 3, 3) and links2.shape == (n, 8, 8, 3, 3)
+    assert np.all(coords.sum(axis=1) % 2 == 0), "M_pc lives on even sites (R8)"
+    out = np.empty((n, Ls, 4, 3), dtype=np.complex128)
+    rc = lib().oracle_mpc_sites(_L(L), ctypes.c_int(Ls), ctypes.c_double(M5), ctypes.c_double(mass), ctypes.c_int64(n),
+                                _p(coords), _p(self_), _p(nbr2), _p(links1), _p(links2), _p(out), ctypes.c_int(int(dagger)))
+    if rc != 0:
+        raise RuntimeError("oracle_mpc_sites: singular M_oo")
     return out

@@ -1,6 +1,7 @@
 """Build libdwf.so (the C-ABI CUDA library) in-tree for sm_100a with nvcc."""
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 
@@ -8,14 +9,13 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdwf.so")
 SOURCES = ["dwf_api.cu"]
-HEADERS = ["dwf_vec.cuh", "dwf_hop.cuh", "dwf_aux.cuh"]
 
 
 def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(HERE, "..", "include", "dwf.h")]
+    deps = glob.glob(os.path.join(CSRC, "*.cu*")) + [os.path.join(HERE, "..", "include", "dwf.h"), os.path.abspath(__file__)]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

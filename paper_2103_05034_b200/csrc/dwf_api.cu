@@ -19,6 +19,10 @@
 
 using namespace dwf;
 
+static const int MAX_RED_BLOCKS = 2048;
+static const int MAX_NRHS = 64;
+static const int SCAL_DOUBLES = 1 << 16;
+
 struct dwf_ctx {
     int L[4], Ls, prec;
     double M5, mass;
@@ -32,10 +36,13 @@ struct dwf_ctx {
     int* inv_lex;         // [V4]: lexicographic site -> index within its parity (built on first use by dwf_convert)
     bool have_gauge;
     void* ws; size_t ws_bytes;
-    double* partial;      // reduction partials [MAX_RED_BLOCKS][64][2]
+    double* partial;      // reduction partials [blocks][nrhs][2]
+    size_t partial_doubles;   // its size: covers blas_blocks(nrhs) * nrhs * 2 for every nrhs <= MAX_NRHS
     double* scal;         // device scalars (reduction results, CG history)
     double* scal_host;    // pinned mirror
-    int sm_count;
+    int sm_count, device;
+    bool no_fuse_moo, no_fuse_norm;   // DWF_NO_FUSE_MOOINV / DWF_NO_FUSE_NORM, read once at dwf_create (the unfused reference path)
+    int cg_graph;         // DWF_CG_GRAPH, read once at dwf_create
     long long blk_sites;  // sites per parity in one lattice block of the native site order
     int tile_sites;       // sites per parity in one tile of the native site order (0: lattice is not made of whole tiles)
     int sg_shift;         // block order [site group][rhs][site in group]: log2(group size)
@@ -44,9 +51,6 @@ struct dwf_ctx {
     char err[256];
 };
 
-static const int MAX_RED_BLOCKS = 2048;
-static const int MAX_NRHS = 64;
-static const int SCAL_DOUBLES = 1 << 16;
 
 #define FAIL(h, code, ...) do { snprintf((h)->err, sizeof((h)->err), __VA_ARGS__); return (code); } while (0)
 #define CUDA_TRY(h, call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) \
@@ -64,6 +68,16 @@ static inline long long half_groups(const dwf_ctx* h, int nrhs) {
 }
 static inline int block_groups(const dwf_ctx* h) { return 12 * h->Ls / vl(h); }   // groups per (site, rhs) block
 static inline int run_groups(const dwf_ctx* h) { return block_groups(h) << h->sg_shift; }   // groups per contiguous run of one rhs
+
+// BLAS-1 launch geometry: (blocks * 256) % period == 0 (period = groups per site group = run_groups * nrhs) so that each
+// thread keeps one rhs for its whole grid-stride loop.  `unit` may exceed MAX_RED_BLOCKS (wide blocks x many rhs):
+// h->partial is sized for that at dwf_create.
+static long long blas_unit(long long period) { return period / std::gcd(period, 256LL); }
+static long long blas_blocks_for(long long unit, long long want) {
+    long long blocks = std::max<long long>(unit, (want / unit) * unit);
+    if (blocks > MAX_RED_BLOCKS) blocks = std::max<long long>(unit, (MAX_RED_BLOCKS / unit) * unit);
+    return blocks;
+}
 
 // ------------------------------------------------------------------------------------------------
 // Index tables.  Native site order within a parity: 4D blocks of BLK^4 sites in lexicographic block
@@ -161,17 +175,26 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
         delete h; return DWF_ECUDA;
     }
+    h->device = dev;
+    h->no_fuse_moo = getenv("DWF_NO_FUSE_MOOINV") != nullptr;
+    h->no_fuse_norm = getenv("DWF_NO_FUSE_NORM") != nullptr;
+    { const char* genv = getenv("DWF_CG_GRAPH"); h->cg_graph = genv ? atoi(genv) : 0; }
     std::vector<int> lex, nbr;
     build_tables(h, lex, nbr);
     h->rhs_chunk = 1;      // measured on B200 (16^3x32x16 fp32): 1 is fastest (132 us per rhs at nrhs 12; 4: 142 us): a chunk of c rhs needs c slabs of the lattice in L2
     if (const char* env = getenv("DWF_RHS_CHUNK")) h->rhs_chunk = std::max(1, atoi(env));
+    h->partial_doubles = (size_t)MAX_RED_BLOCKS * MAX_NRHS * 2;
+    for (int n = 1; n <= MAX_NRHS; n++) {                    // worst case of blas_blocks(): one unit of blocks larger than MAX_RED_BLOCKS
+        const long long unit = blas_unit((long long)run_groups(h) * n);
+        h->partial_doubles = std::max(h->partial_doubles, (size_t)blas_blocks_for(unit, MAX_RED_BLOCKS) * n * 2);
+    }
     const size_t gbytes = (size_t)2 * h->V4h * 72 * real_bytes(h);
     const size_t glbytes = (size_t)2 * h->V4h * (144 * real_bytes(h) + 16);
     bool ok = cudaMalloc(&h->gauge, gbytes) == cudaSuccess
            && (h->tile_sites == 0 || (cudaMalloc(&h->glinks, glbytes) == cudaSuccess && cudaMemset(h->glinks, 0, glbytes) == cudaSuccess))
            && cudaMalloc((void**)&h->nbr, nbr.size() * sizeof(int)) == cudaSuccess
            && cudaMalloc((void**)&h->lex, lex.size() * sizeof(int)) == cudaSuccess
-           && cudaMalloc((void**)&h->partial, (size_t)MAX_RED_BLOCKS * MAX_NRHS * 2 * sizeof(double)) == cudaSuccess
+           && cudaMalloc((void**)&h->partial, h->partial_doubles * sizeof(double)) == cudaSuccess
            && cudaMalloc((void**)&h->scal, SCAL_DOUBLES * sizeof(double)) == cudaSuccess
            && cudaMallocHost((void**)&h->scal_host, SCAL_DOUBLES * sizeof(double)) == cudaSuccess
            && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
@@ -337,8 +360,12 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
         using TG = TileGeom<R, LS, TSV>; \
         auto kern = hop_tile_kernel<R, LS, TSV, DAG, true, SELF, G5, AX, MOO, NRM>; \
         if (NRM && k.norm_count) *k.norm_count = a.nitems * (TG::THREADS / 32); \
-        cudaError_t e_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TG::SMEM_BYTES); \
-        if (e_ != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e_)); \
+        static unsigned long long attr_done = 0;              /* per kernel instantiation: devices whose attribute is set */ \
+        if (!((attr_done >> (h->device & 63)) & 1ull)) { \
+            cudaError_t e_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TG::SMEM_BYTES); \
+            if (e_ != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e_)); \
+            attr_done |= 1ull << (h->device & 63); \
+        } \
         const long long ctas = std::min<long long>(a.nitems, (long long)h->sm_count * TG::MIN_CTAS); \
         kern<<<(unsigned)ctas, TG::THREADS, TG::SMEM_BYTES, st>>>(a); } while (0)
 #define HOPM(LS) \
@@ -429,7 +456,7 @@ static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, co
 static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp);
 static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs, double* norm_out = nullptr) {
     // K1: tmp_o = M_oo^-1 Dhop_oe in -- one launch when the tiled kernel applies (M_oo^-1 fused as its epilogue)
-    const bool fused = tiled_ok(h) && !getenv("DWF_NO_FUSE_MOOINV");
+    const bool fused = tiled_ok(h) && !h->no_fuse_moo;
     HopCall k1{};
     k1.mode = fused ? HM_HOP_MOOINV : HM_HOP; k1.dag = dag; k1.nslots = 1; k1.parity0 = 1; k1.nrhs = nrhs;
     k1.in_hop[0] = in; k1.out[0] = tmp; k1.c_hop = 1.0; k1.mass = h->mass;
@@ -439,9 +466,9 @@ static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, 
     k2.mode = HM_HOP_SELF; k2.dag = dag; k2.nslots = 1; k2.parity0 = 0; k2.nrhs = nrhs;
     k2.in_hop[0] = tmp; k2.in_self[0] = in; k2.out[0] = out; k2.c_hop = -0.25; k2.mass = h->mass;
     long long nparts = 0;
-    const long long max_parts = (long long)MAX_RED_BLOCKS * MAX_NRHS;
+    const long long max_parts = (long long)(h->partial_doubles / 2);
     const long long tile_warps = h->tile_sites ? (h->V4h / h->tile_sites) * ((long long)h->tile_sites * h->Ls / vl(h) / 32) : 0;
-    const bool fuse_norm = norm_out && fused && nrhs == 1 && !dag && tile_warps <= max_parts && !getenv("DWF_NO_FUSE_NORM");
+    const bool fuse_norm = norm_out && fused && nrhs == 1 && !dag && tile_warps <= max_parts && !h->no_fuse_norm;
     if (fuse_norm) { k2.norm_partial = h->partial; k2.norm_count = &nparts; }
     if (int rc = launch_hop(h, k2)) return rc;
     if (!norm_out) return DWF_OK;
@@ -477,7 +504,7 @@ static int apply_checked(dwf_ctx* h, int op, const void* in, void* out, int nrhs
             const size_t hb = half_bytes(h, nrhs);
             if (int rc = need_ws(h, 2 * hb)) return rc;
             void* t1 = h->ws; void* t2 = (char*)h->ws + hb;
-            const bool fusedk = tiled_ok(h) && !getenv("DWF_NO_FUSE_MOOINV");
+            const bool fusedk = tiled_ok(h) && !h->no_fuse_moo;
             auto hop_moo = [&](int parity_out, const void* src, void* dst, bool with_moo) -> int {   // dst_p = [M_pp^-1] Dhop src_{1-p}
                 HopCall k{}; k.mode = (with_moo && fusedk) ? HM_HOP_MOOINV : HM_HOP; k.dag = dag; k.nslots = 1; k.parity0 = parity_out; k.nrhs = nrhs;
                 k.in_hop[0] = src; k.out[0] = dst; k.c_hop = 1.0; k.mass = h->mass;
@@ -574,6 +601,17 @@ extern "C" int dwf_chebyshev_subspace(dwf_handle h, int m, double lambda_lo, dou
     if (int rc = need_ws(h, 3 * fb)) return rc;
     // first pass straight into phi_0 (dwf_chebyshev uses workspace fields 0 and 1)
     if (int rc = dwf_chebyshev(h, m, lambda_lo, lambda_max, eta, phi, nrhs)) return rc;
+    // Outside [lambda_lo, lambda_max] T_m grows as cosh(m acosh|x|) (Fig. 2: 1e8 for the paper's parameters, but
+    // 1e137 for m = 600, lambda_lo = 4): no normalisation is applied (R14), so an overflow of the field's precision is
+    // reported instead of returning inf/nan vectors.
+    auto check_finite = [&](const void* f, const char* what) -> int {
+        double n2[MAX_NRHS];
+        if (int rc = dwf_norm2(h, f, n2, nrhs, 0)) return rc;
+        for (int q = 0; q < nrhs; q++) if (!std::isfinite(n2[q]))
+            FAIL(h, DWF_ERANGE, "%s overflowed %s (rhs %d): lower m or raise lambda_lo, or use an fp64 handle", what, h->prec == DWF_F32 ? "fp32" : "fp64", q);
+        return DWF_OK;
+    };
+    if (int rc = check_finite(phi, "first-pass filter T_m")) return rc;
     if (nvec == 1) return DWF_OK;
     void* w = h->ws; void* A = (char*)h->ws + fb; void* B = (char*)h->ws + 2 * fb;
     const double alpha = 2.0 / lambda_max, beta = 1.0;                          // X' = alpha H^2 - beta
@@ -591,7 +629,7 @@ extern "C" int dwf_chebyshev_subspace(dwf_handle h, int m, double lambda_lo, dou
         if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, 2.0 * alpha, tk, -2.0 * beta, tkm1, -1.0)) return rc;
         tkm1 = tk; tk = dst;
     }
-    return DWF_OK;
+    return check_finite((char*)phi + (size_t)(nvec - 1) * fb, "second-pass recurrence");   // lambda_max below the true one: |x| > 1
 }
 
 // Chebyshev smoother (eq. 24-25):
@@ -630,12 +668,15 @@ extern "C" int dwf_chebyshev_smoother(dwf_handle h, int N, double a, double b, c
     if (int rc = full_op(h, HM_HOP_SELF, true, -0.5, h->mass, r, v, nrhs)) return rc;           // v = D_DW^dag r
     CUDA_TRY(h, cudaMemsetAsync(out, 0, fb, h->stream));
     if (int rc = add(0.5 * c[0], v)) return rc;
+    // c_N = (2/N) sum_k cos(N theta_k)/y_k vanishes identically (cos(N theta_k) = cos(pi (k + 1/2)) = 0): the sum of eq. 24
+    // stops at j = N-1 and the last recurrence step (two operator applies) is not needed.
+    if (N == 1) return DWF_OK;
     const double alpha = 2.0 / (b - a), beta = (b + a) / (b - a);
     if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, v, w, nrhs)) return rc;
     if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, A, nrhs, alpha, v, -beta, v, 0.0)) return rc;
     if (int rc = add(c[1], A)) return rc;
     const void* tkm1 = v; void* tk = A;
-    for (int k = 1; k < N; k++) {
+    for (int k = 1; k < N - 1; k++) {
         void* dst = (k == 1) ? B : (void*)tkm1;
         if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, tk, w, nrhs)) return rc;
         if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, 2.0 * alpha, tk, -2.0 * beta, tkm1, -1.0)) return rc;
@@ -662,8 +703,11 @@ extern "C" int dwf_power_lambda_max(dwf_handle h, int iters, void* v, double* la
     for (int i = 0; i < iters; i++) {
         if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, cur, u, 1)) return rc;
         double nu = 0, nv = 0;
-        if (int rc = dwf_norm2(h, u, &nu, 1, 0)) return rc;
-        if (int rc = dwf_norm2(h, cur, &nv, 1, 0)) return rc;
+        if (int rc = reduce_to(h, true, u, nullptr, 1, 0, h->scal, 1, 1)) return rc;
+        if (int rc = reduce_to(h, true, cur, nullptr, 1, 0, h->scal + 1, 1, 1)) return rc;
+        CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+        nu = h->scal_host[0]; nv = h->scal_host[1];
         if (!(nv > 0.0) || !(nu > 0.0)) FAIL(h, DWF_EINVAL, "power method: zero vector");
         lam = nu / nv;
         if (lambda_hist_host) lambda_hist_host[i] = lam;
@@ -680,12 +724,8 @@ extern "C" int dwf_power_lambda_max(dwf_handle h, int iters, void* v, double* la
 // BLAS-1
 // ------------------------------------------------------------------------------------------------
 static unsigned blas_blocks(const dwf_ctx* h, long long ngroups, long long period) {
-    // (blocks * 256) % period == 0 (period = groups per site = BS * nrhs) so that each thread keeps one rhs
-    const long long unit = period / std::gcd(period, 256LL);
-    long long want = std::min<long long>((ngroups + 255) / 256, (long long)h->sm_count * 8);
-    long long blocks = std::max<long long>(unit, (want / unit) * unit);
-    if (blocks > MAX_RED_BLOCKS) blocks = std::max<long long>(unit, (MAX_RED_BLOCKS / unit) * unit);
-    return (unsigned)blocks;
+    const long long want = std::min<long long>((ngroups + 255) / 256, (long long)h->sm_count * 8);
+    return (unsigned)blas_blocks_for(blas_unit(period), want);
 }
 
 static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp) {
@@ -806,8 +846,7 @@ static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int ite
     // The host loop only enqueues (alpha, beta live on the device).  DWF_CG_GRAPH=1 captures the whole solve into a
     // CUDA graph and launches it as one unit; measured on B200 (8^4x16: 7037 vs 7388 it/s, 16^3x32x16: no change)
     // the plain stream launches are already back to back, so the graph is off by default.
-    const char* genv = getenv("DWF_CG_GRAPH");
-    const bool use_graph = genv && atoi(genv) != 0 && iters > 0;
+    const bool use_graph = h->cg_graph != 0 && iters > 0;
     int rc;
     if (use_graph) {
         cudaStream_t user = h->stream;
@@ -847,6 +886,65 @@ extern "C" int dwf_cg_normal(dwf_handle h, const void* b, void* x, int iters, in
 }
 
 // ------------------------------------------------------------------------------------------------
+// BiCGSTAB on the Pauli-Villars preconditioned operator A = M_PV^dag M = D_PV^dag D_DW (PAPER.md L101-107,
+// Table V, ref. [31] van der Vorst).  Full native fields, one right-hand side; x holds x_0 on entry.
+//   r_0 = b - A x_0, rhat0 = r_0, p_1 = r_0;  per iteration i:
+//   rho_i = <rhat0, r_{i-1}>; p_i = r_{i-1} + beta_i (p_{i-1} - omega_{i-1} v_{i-1}); v_i = A p_i; alpha_i = rho_i/<rhat0, v_i>;
+//   s = r_{i-1} - alpha_i v_i; t = A s; omega_i = <t,s>/<t,t>; x_i = x_{i-1} + alpha_i p_i + omega_i s; r_i = s - omega_i t.
+// The host loop only enqueues: every scalar stays on the device (dwf_aux.cuh, slots of 8 doubles per iteration); 12 launches
+// and 2 applies of A (4 stencil launches) per iteration.  Workspace: r(=s), rhat0, p, v, t + the scratch of A = 6 full fields.
+// ------------------------------------------------------------------------------------------------
+template <typename R>
+static int bicgstab_t(dwf_ctx* h, const void* b, void* x, int iters) {
+    using G = typename Prec<R>::G;
+    const size_t fb = 2 * half_bytes(h, 1);
+    const long long ng = 2 * half_groups(h, 1);
+    G* r = (G*)h->ws; G* rhat = (G*)((char*)h->ws + fb); G* p = (G*)((char*)h->ws + 2 * fb);
+    G* v = (G*)((char*)h->ws + 3 * fb); G* t = (G*)((char*)h->ws + 4 * fb); void* scratch = (char*)h->ws + 5 * fb;
+    auto A = [&](const void* in, void* out) -> int {                            // out = D_PV^dag (D_DW in)
+        if (int rc = full_op(h, HM_HOP_SELF, false, -0.5, h->mass, in, scratch, 1)) return rc;
+        return full_op(h, HM_HOP_SELF, true, -0.5, 1.0, scratch, out, 1);
+    };
+    const unsigned blocks = (unsigned)std::min<long long>((ng + 255) / 256, (long long)h->sm_count * 8);
+    cudaStream_t st = h->stream;
+    double* S = h->scal;                                                        // slot(i) = S + 8 i
+    if (int rc = A(x, v)) return rc;
+    bicg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, v, r, rhat, ng, h->partial); LAUNCH_CHECK(h);
+    reduce_final4_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, S, 7, -1, 8 + 0, 8 + 1); LAUNCH_CHECK(h);   // |r_0|^2 ; rho_1
+    for (int i = 1; i <= iters; i++) {
+        double* slot = S + 8 * (size_t)i;
+        bicg_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, v, ng, slot - 8, slot, i == 1); LAUNCH_CHECK(h);
+        if (int rc = A(p, v)) return rc;
+        inner_pair_kernel<R><<<blocks, 256, 0, st>>>(rhat, v, ng, h->partial); LAUNCH_CHECK(h);
+        reduce_final4_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, slot, 2, 3, -1, -1); LAUNCH_CHECK(h);    // <rhat0, v_i>
+        bicg_s_kernel<R><<<blocks, 256, 0, st>>>(r, v, ng, slot); LAUNCH_CHECK(h);
+        if (int rc = A(r, t)) return rc;
+        inner_pair_kernel<R><<<blocks, 256, 0, st>>>(t, r, ng, h->partial); LAUNCH_CHECK(h);
+        reduce_final4_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, slot, 4, 5, 6, -1); LAUNCH_CHECK(h);     // <t,s>, <t,t>
+        bicg_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, t, rhat, ng, slot, h->partial); LAUNCH_CHECK(h);
+        reduce_final4_kernel<<<1, 256, 0, st>>>(h->partial, (int)blocks, slot, 7, -1, 8 + 0, 8 + 1); LAUNCH_CHECK(h);   // |r_i|^2 ; rho_{i+1}
+    }
+    return DWF_OK;
+}
+
+extern "C" int dwf_bicgstab_pv(dwf_handle h, const void* b, void* x, int iters, double* resid2_hist_host) {
+    if (!h) return DWF_EINVAL;
+    if (iters < 0 || 8 * ((long long)iters + 2) > SCAL_DOUBLES) FAIL(h, DWF_EINVAL, "iters must be in [0,%d]", SCAL_DOUBLES / 8 - 2);
+    if (int rc = check_field(h, b, "b")) return rc;
+    if (int rc = check_field(h, x, "x")) return rc;
+    if (b == x) FAIL(h, DWF_EINVAL, "b == x");
+    if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    if (int rc = need_ws(h, 12 * half_bytes(h, 1))) return rc;
+    if ((size_t)std::min<long long>((2 * half_groups(h, 1) + 255) / 256, (long long)h->sm_count * 8) * 4 > h->partial_doubles)
+        FAIL(h, DWF_EUNSUPPORTED, "reduction scratch too small");
+    if (int rc = h->prec == DWF_F32 ? bicgstab_t<float>(h, b, x, iters) : bicgstab_t<double>(h, b, x, iters)) return rc;
+    CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, h->scal, 8 * ((size_t)iters + 1) * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (resid2_hist_host) for (int i = 0; i <= iters; i++) resid2_hist_host[i] = h->scal_host[8 * (size_t)i + 7];
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Complete red-black solve of D_DW psi = eta (Table V, eq. 9), nrhs = 1:
 //   eta'_e = eta_e - M_eo M_oo^-1 eta_o ;  CGNR: M_pc^dag M_pc psi_e = M_pc^dag eta'_e (stop: |r_k| <= tol |r_0|, tested
 //   every 10 iterations) ;  psi_o = M_oo^-1 (eta_o - M_oe psi_e) ;  M_eo = M_oe = -1/2 Dhop.
@@ -863,6 +961,18 @@ extern "C" int dwf_solve(dwf_handle h, const void* eta, void* psi, double tol, i
     if (int rc = need_ws(h, 8 * hb)) return rc;
     const char* eta_e = (const char*)eta; const char* eta_o = eta_e + hb;
     char* psi_e = (char*)psi; char* psi_o = psi_e + hb;
+    {                                                         // eta = 0: psi = 0 (CG on a zero right-hand side would divide 0 by 0)
+        double ne0 = 0;
+        if (int rc = dwf_norm2(h, eta, &ne0, 1, 0)) return rc;
+        if (!(ne0 > 0.0)) {
+            if (ne0 != 0.0) FAIL(h, DWF_EINVAL, "eta is not finite");
+            CUDA_TRY(h, cudaMemsetAsync(psi, 0, 2 * hb, h->stream));
+            CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+            if (iters_host) *iters_host = 0;
+            if (relres_host) *relres_host = 0.0;
+            return DWF_OK;
+        }
+    }
     char* B = (char*)h->ws + 5 * hb; char* T = (char*)h->ws + 6 * hb; char* W = (char*)h->ws + 7 * hb;
     const double half[2] = {0.5, 0.0};
     auto hop_to = [&](int parity_out, const void* in, void* out) -> int {       // out_p = Dhop in_{1-p}
@@ -987,7 +1097,8 @@ extern "C" int dwf_solve_mixed(dwf_handle h64, dwf_handle h32, const void* eta, 
 
 // ------------------------------------------------------------------------------------------------
 // End-to-end apply from host canonical arrays (bench.py's e2e leg): H2D, import, apply, export, D2H.
-// Workspace use: [0, F) canonical staging / native out, [F, 2F) native in / canonical out, [2F, 2F+H) Schur tmp
+// Workspace use: [0, F) canonical staging / native out, [F, 2F) native in / canonical out, [2F, ...) the operator's own scratch
+// (SCHUR_EO: 1 half field, SCHUR_EO_ALT and MPVDAG_M: 2)
 // ------------------------------------------------------------------------------------------------
 extern "C" int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* out_host, int nrhs) {
     if (!h) return DWF_EINVAL;
@@ -995,10 +1106,11 @@ extern "C" int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* o
     if (!in_host || !out_host) FAIL(h, DWF_EINVAL, "NULL host pointer");
     const int base = op & ~DWF_DAGGER;
     const bool halfop = (base == DWF_SCHUR_EO || base == DWF_MEE || base == DWF_MOOINV || base == DWF_SCHUR_EO_ALT);
-    if (!halfop && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
-    if (base == DWF_SCHUR_EO && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
+    if (base != DWF_MEE && base != DWF_MOOINV && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
     const size_t hb = half_bytes(h, nrhs), fb = 2 * hb;
-    if (int rc = need_ws(h, 5 * hb)) return rc;
+    // scratch of the operator itself, behind the two staging fields
+    const size_t op_ws = (base == DWF_SCHUR_EO) ? hb : (base == DWF_SCHUR_EO_ALT || base == DWF_MPVDAG_M) ? 2 * hb : 0;
+    if (int rc = need_ws(h, 2 * fb + op_ws)) return rc;
     char* A = (char*)h->ws; char* B = A + fb; void* tmp = A + 2 * fb;
     void* saved_ws = h->ws; size_t saved_n = h->ws_bytes;
     CUDA_TRY(h, cudaMemcpyAsync(A, in_host, fb, cudaMemcpyHostToDevice, h->stream));
@@ -1007,7 +1119,7 @@ extern "C" int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* o
     void* nat_in = B; void* nat_out = halfop ? (void*)(B + hb) : (void*)A; void* can_out = halfop ? (void*)A : (void*)B;
     int rc = dwf_import(h, A, nat_in, nrhs, halfop ? 0 : -1);
     if (!rc) {
-        h->ws = tmp; h->ws_bytes = hb;                 // Schur scratch lives behind the two staging buffers
+        h->ws = tmp; h->ws_bytes = op_ws;              // the operator's scratch lives behind the two staging buffers
         rc = apply_checked(h, op, nat_in, nat_out, nrhs);
         h->ws = saved_ws; h->ws_bytes = saved_n;
     }

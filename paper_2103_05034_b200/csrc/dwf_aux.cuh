@@ -305,7 +305,7 @@ cg_update_xr_kernel(typename Prec<R>::G* x, typename Prec<R>::G* r, const typena
     const long long stride = (long long)gridDim.x * blockDim.x;
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int rhs = (int)((e / BS) % nrhs);
-    const R alpha = (R)(rr[rhs] / pAp[rhs]);
+    const R alpha = pAp[rhs] != 0.0 ? (R)(rr[rhs] / pAp[rhs]) : R(0);       // zero or converged right-hand side: frozen
     double sre = 0, sim = 0;
     for (; e < ngroups; e += stride) {
         const CV<V> pp = unpack(ldg_nc(p + e)), qq = unpack(ldg_nc(q + e));
@@ -326,13 +326,171 @@ cg_update_p_kernel(typename Prec<R>::G* p, const typename Prec<R>::G* __restrict
     const long long stride = (long long)gridDim.x * blockDim.x;
     long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int rhs = (int)((e / BS) % nrhs);
-    const R beta = (R)(rr_new[rhs] / rr_old[rhs]);
+    const R beta = rr_old[rhs] != 0.0 ? (R)(rr_new[rhs] / rr_old[rhs]) : R(0);
     for (; e < ngroups; e += stride) {
         const CV<V> rv = unpack(ldg_nc(r + e));
         CV<V> pp = unpack(p[e]);
         pp.re = vfma(beta, pp.re, rv.re); pp.im = vfma(beta, pp.im, rv.im);
         p[e] = pack(pp);
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// N4. BiCGSTAB vector updates (van der Vorst, PAPER.md ref. [31] L671; Table V), one right-hand side, full fields.
+// All scalars live on the device in per-iteration slots of 8 doubles (dwf_bicgstab_pv in dwf_api.cu):
+//   slot(i) = { rho_i (re, im), <rhat0, v_i> (re, im), <t_i, s_i> (re, im), <t_i, t_i>, |r_i|^2 },   rho_i = <rhat0, r_{i-1}>
+//   alpha_i = rho_i / <rhat0, v_i>,  omega_i = <t_i, s_i> / <t_i, t_i>,  beta_i = (rho_i / rho_{i-1}) (alpha_{i-1} / omega_{i-1}).
+// A zero denominator (zero or exactly converged right-hand side) freezes the iteration: the coefficient is 0.
+// ------------------------------------------------------------------------------------------------
+struct cd { double re, im; };
+__device__ __forceinline__ cd cd_div(cd a, cd b) {
+    const double n = b.re * b.re + b.im * b.im;
+    if (n == 0.0) return {0.0, 0.0};
+    return {(a.re * b.re + a.im * b.im) / n, (a.im * b.re - a.re * b.im) / n};
+}
+__device__ __forceinline__ cd cd_mul(cd a, cd b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ cd bicg_alpha(const double* slot) { return cd_div({slot[0], slot[1]}, {slot[2], slot[3]}); }
+__device__ __forceinline__ cd bicg_omega(const double* slot) {
+    return slot[6] != 0.0 ? cd{slot[4] / slot[6], slot[5] / slot[6]} : cd{0.0, 0.0};
+}
+// y += a x  for complex a, lane vectors
+template <typename R, typename V> __device__ __forceinline__ void caxpy(CV<V>& y, R are, R aim, const CV<V>& x) {
+    y.re = vfnma(aim, x.im, vfma(are, x.re, y.re));
+    y.im = vfma(aim, x.re, vfma(are, x.im, y.im));
+}
+
+// Fixed-order combine of per-thread sums (4 components) into per-block partials partial[blockIdx.x * 4 + c]: a binary tree over
+// the 256 threads in shared memory (deterministic).
+__device__ __forceinline__ void block_combine4(double a0, double a1, double a2, double a3, double* partial) {
+    __shared__ double s4[4][256];
+    const int t = threadIdx.x;
+    s4[0][t] = a0; s4[1][t] = a1; s4[2][t] = a2; s4[3][t] = a3;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (t < w) { s4[0][t] += s4[0][t + w]; s4[1][t] += s4[1][t + w]; s4[2][t] += s4[2][t + w]; s4[3][t] += s4[3][t + w]; }
+        __syncthreads();
+    }
+    if (t < 4) partial[(size_t)blockIdx.x * 4 + t] = s4[t][0];
+}
+// out[c] = sum over blocks of partial[k*4 + c] for the components c with out_idx[c] >= 0 (written to out[out_idx[c]])
+__global__ void __launch_bounds__(256)
+reduce_final4_kernel(const double* __restrict__ partial, int nblocks, double* out, int i0, int i1, int i2, int i3) {
+    __shared__ double s4[4][256];
+    const int t = threadIdx.x;
+    double a[4] = {0, 0, 0, 0};
+    for (int k = t; k < nblocks; k += 256)
+#pragma unroll
+        for (int c = 0; c < 4; c++) a[c] += partial[(size_t)k * 4 + c];
+#pragma unroll
+    for (int c = 0; c < 4; c++) s4[c][t] = a[c];
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if (t < w) {
+#pragma unroll
+            for (int c = 0; c < 4; c++) s4[c][t] += s4[c][t + w];
+        }
+        __syncthreads();
+    }
+    if (t == 0) {
+        const int idx[4] = {i0, i1, i2, i3};
+#pragma unroll
+        for (int c = 0; c < 4; c++) if (idx[c] >= 0) out[idx[c]] = s4[c][0];
+    }
+}
+
+// partials {Re<x,y>, Im<x,y>, <x,x>, 0}
+template <typename R>
+__global__ void __launch_bounds__(256)
+inner_pair_kernel(const typename Prec<R>::G* __restrict__ x, const typename Prec<R>::G* __restrict__ y, long long ngroups, double* partial) {
+    using V = typename Prec<R>::V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double sre = 0, sim = 0, nre = 0, nim = 0;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        const CV<V> xx = unpack(ldg_nc(x + e)), yy = unpack(ldg_nc(y + e));
+        acc_inner(sre, sim, xx, yy);
+        acc_inner(nre, nim, xx, xx);
+    }
+    block_combine4(sre, sim, nre, 0.0, partial);
+}
+
+// init: r = b - q (q = A x_0), rhat0 = r, p = v = 0; partials {|r|^2, 0, |r|^2, 0} (rho_1 = <rhat0, r_0> = |r_0|^2)
+template <typename R>
+__global__ void __launch_bounds__(256)
+bicg_init_kernel(const typename Prec<R>::G* __restrict__ b, const typename Prec<R>::G* __restrict__ q, typename Prec<R>::G* r,
+                 typename Prec<R>::G* rhat, long long ngroups, double* partial) {
+    using V = typename Prec<R>::V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    double sre = 0, sim = 0;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        const CV<V> rr = csub(unpack(ldg_nc(b + e)), unpack(ldg_nc(q + e)));
+        r[e] = pack(rr); rhat[e] = pack(rr);
+        acc_inner(sre, sim, rr, rr);
+    }
+    block_combine4(sre, 0.0, sre, 0.0, partial);
+}
+
+// p = r + beta (p - omega_{i-1} v);  first iteration: p = r
+template <typename R>
+__global__ void __launch_bounds__(256)
+bicg_p_kernel(typename Prec<R>::G* p, const typename Prec<R>::G* __restrict__ r, const typename Prec<R>::G* __restrict__ v,
+              long long ngroups, const double* __restrict__ slot_prev, const double* __restrict__ slot, int first) {
+    using V = typename Prec<R>::V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    cd beta = {0, 0}, om = {0, 0};
+    if (!first) {
+        om = bicg_omega(slot_prev);
+        beta = cd_mul(cd_div({slot[0], slot[1]}, {slot_prev[0], slot_prev[1]}), cd_div(bicg_alpha(slot_prev), om));
+    }
+    const R bre = (R)beta.re, bim = (R)beta.im, ore = (R)(-om.re), oim = (R)(-om.im);
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        CV<V> out = unpack(ldg_nc(r + e));
+        if (!first) {
+            CV<V> d = unpack(p[e]);
+            caxpy<R>(d, ore, oim, unpack(ldg_nc(v + e)));          // p - omega v
+            caxpy<R>(out, bre, bim, d);
+        }
+        p[e] = pack(out);
+    }
+}
+
+// s = r - alpha_i v   (in place: s overwrites r)
+template <typename R>
+__global__ void __launch_bounds__(256)
+bicg_s_kernel(typename Prec<R>::G* r, const typename Prec<R>::G* __restrict__ v, long long ngroups, const double* __restrict__ slot) {
+    using V = typename Prec<R>::V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const cd al = bicg_alpha(slot);
+    const R are = (R)(-al.re), aim = (R)(-al.im);
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        CV<V> s = unpack(r[e]);
+        caxpy<R>(s, are, aim, unpack(ldg_nc(v + e)));
+        r[e] = pack(s);
+    }
+}
+
+// x += alpha_i p + omega_i s ;  r = s - omega_i t  (in place over s);  partials {|r|^2, 0, Re<rhat0, r>, Im<rhat0, r>}
+template <typename R>
+__global__ void __launch_bounds__(256)
+bicg_xr_kernel(typename Prec<R>::G* x, typename Prec<R>::G* sr, const typename Prec<R>::G* __restrict__ p,
+               const typename Prec<R>::G* __restrict__ t, const typename Prec<R>::G* __restrict__ rhat, long long ngroups,
+               const double* __restrict__ slot, double* partial) {
+    using V = typename Prec<R>::V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    const cd al = bicg_alpha(slot), om = bicg_omega(slot);
+    const R are = (R)al.re, aim = (R)al.im, ore = (R)om.re, oim = (R)om.im;
+    double nre = 0, nim = 0, hre = 0, him = 0;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < ngroups; e += stride) {
+        CV<V> xx = unpack(x[e]);
+        CV<V> s = unpack(sr[e]);
+        caxpy<R>(xx, are, aim, unpack(ldg_nc(p + e)));
+        caxpy<R>(xx, ore, oim, s);
+        x[e] = pack(xx);
+        caxpy<R>(s, (R)(-om.re), (R)(-om.im), unpack(ldg_nc(t + e)));
+        sr[e] = pack(s);
+        acc_inner(nre, nim, s, s);
+        acc_inner(hre, him, unpack(ldg_nc(rhat + e)), s);
+    }
+    block_combine4(nre, 0.0, hre, him, partial);
 }
 
 }  // namespace dwf

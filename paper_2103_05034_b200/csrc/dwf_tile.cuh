@@ -222,6 +222,8 @@ hop_tile_kernel(const HopArgs<R> a) {
                     __threadfence_block();                     // this warp's reads of the buffers are performed before it counts itself done
                     const unsigned prev = atomicAdd(done_count + buf, 1u);
                     if (prev == (unsigned)((it >> 1) + 1) * NWARPS - 1) {
+                        // generic-proxy accesses of the buffers (reads; the MOO transpose also writes) before the async-proxy refill
+                        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                         if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);
                         if (wn + gridDim.x < a.nitems) { issue_small(wn + gridDim.x, buf); if (NSTI == 2) issue_interior(wn + gridDim.x, buf); }
                     }

@@ -13,7 +13,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libdwf.so")
+# DWF_LIB: load another build of the same library (kernel tuning); the default is the in-tree libdwf.so
+_LIB_PATH = os.environ.get("DWF_LIB") or os.path.join(_HERE, "libdwf.so")
 
 DWF_F32, DWF_F64 = 0, 1
 DWF_DHOP, DWF_DDW, DWF_HDW, DWF_DPV, DWF_SCHUR_EO, DWF_MEE, DWF_MOOINV, DWF_MPVDAG_M, DWF_SCHUR_EO_ALT = range(9)
@@ -53,6 +54,7 @@ _SIGNATURES = {
                                           ctypes.POINTER(ctypes.c_double)]),
     "dwf_cg_normal": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
                                      ctypes.POINTER(ctypes.c_double)]),
+    "dwf_bicgstab_pv": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]),
     "dwf_solve": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_double, ctypes.c_int,
                                  ctypes.POINTER(ctypes.c_int), ctypes.POINTER(ctypes.c_double)]),
     "dwf_convert": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]),
@@ -73,8 +75,15 @@ def exported_symbols():
     return sorted(_SIGNATURES)
 
 
+DWF_EINVAL, DWF_ENOGAUGE, DWF_ENOMEM, DWF_ECUDA, DWF_EUNSUPPORTED, DWF_ENOWORKSPACE, DWF_ERANGE = -1, -2, -3, -4, -5, -6, -7
+
+
 class DwfError(RuntimeError):
-    pass
+    """A negative return code of the C ABI; `.code` is that code."""
+
+    def __init__(self, msg, code=None):
+        super().__init__(msg)
+        self.code = code
 
 
 _lib = None
@@ -121,7 +130,7 @@ class Dwf:
     # -- plumbing -------------------------------------------------------------------------------
     def _check(self, rc: int):
         if rc != 0:
-            raise DwfError(f"libdwf error {rc}: {self.lib.dwf_last_error(self._h).decode()}")
+            raise DwfError(f"libdwf error {rc}: {self.lib.dwf_last_error(self._h).decode()}", rc)
 
     def close(self):
         if self._h is not None:
@@ -250,6 +259,12 @@ class Dwf:
         hist = (ctypes.c_double * ((iters + 1) * nrhs))()
         self._check(self.lib.dwf_cg_normal(self._h, ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), iters, nrhs, hist))
         return [[float(hist[k * nrhs + r]) for r in range(nrhs)] for k in range(iters + 1)]
+
+    def bicgstab_pv(self, b: torch.Tensor, x: torch.Tensor, iters: int):
+        """BiCGSTAB on D_PV^dag D_DW x = b (full fields, nrhs = 1); returns the |r_i|^2 history (iters + 1 values)."""
+        hist = (ctypes.c_double * (iters + 1))()
+        self._check(self.lib.dwf_bicgstab_pv(self._h, ctypes.c_void_p(b.data_ptr()), ctypes.c_void_p(x.data_ptr()), iters, hist))
+        return [float(v) for v in hist]
 
     def solve(self, eta: torch.Tensor, psi: torch.Tensor, tol: float, max_iters: int):
         """D_DW psi = eta by the complete red-black CGNR solve; returns (iterations, true relative residual)."""

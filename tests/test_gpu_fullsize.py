@@ -34,7 +34,7 @@ def _batch_with_samples(rig, nrhs, seed, sample):
 
 
 @pytest.mark.parametrize("prec,nrhs,sample", [("f32", 1, [0]), ("f64", 1, [0]), ("f32", 12, [0, 11]), ("f64", 12, [5]),
-                                              ("f32", 48, [0, 23, 47])])
+                                              ("f32", 48, [0, 23, 47]), ("f64", 48, [7, 47])])
 def test_config2_ddw_hdw(oracle, prec, nrhs, sample):
     rig = Rig(L2, 16, prec, 0.01, seed_U=1002)
     can, fields = _batch_with_samples(rig, nrhs, 2002, sample)
@@ -96,6 +96,33 @@ def _sample_sites(L, n_random, seed):
     return np.array(sorted(set(sites)), dtype=np.int64)
 
 
+def _gather_two_hop(L, psi, U, st):
+    """Two-hop neighbourhoods of the even sites st[n,4] (device) in the layout oracle.mpc_sites expects: indexing only."""
+    dev = st.device
+    n, Ls = st.shape[0], psi.shape[1]
+    Lt_ = torch.tensor(L, device=dev)
+
+    def fetch_psi(c):
+        return psi[0][:, c[:, 3], c[:, 2], c[:, 1], c[:, 0]].permute(1, 0, 2, 3).cpu().numpy().astype(np.complex128)
+
+    def fetch_link(mu, c):
+        return U[mu][c[:, 3], c[:, 2], c[:, 1], c[:, 0]].cpu().numpy().astype(np.complex128)
+    self_ = fetch_psi(st)
+    nbr2 = np.zeros((n, 8, 8, Ls, 4, 3), dtype=np.complex128)
+    links1 = np.zeros((n, 8, 3, 3), dtype=np.complex128)
+    links2 = np.zeros((n, 8, 8, 3, 3), dtype=np.complex128)
+    for mu in range(4):
+        for j, d in enumerate((+1, -1)):
+            y = st.clone(); y[:, mu] = (y[:, mu] + d) % Lt_[mu]
+            links1[:, 2 * mu + j] = fetch_link(mu, st if d > 0 else y)
+            for nu in range(4):
+                for k, e in enumerate((+1, -1)):
+                    z = y.clone(); z[:, nu] = (z[:, nu] + e) % Lt_[nu]
+                    nbr2[:, 2 * mu + j, 2 * nu + k] = fetch_psi(z)
+                    links2[:, 2 * mu + j, 2 * nu + k] = fetch_link(nu, y if e > 0 else z)
+    return self_, nbr2, links1, links2
+
+
 def test_config4_ddw_sampled_and_cg_invariants(oracle):
     import gc
     gc.collect(); torch.cuda.empty_cache()
@@ -134,7 +161,28 @@ def test_config4_ddw_sampled_and_cg_invariants(oracle):
     assert err < TOL_APPLY["f32"], err
     worst = np.max(np.linalg.norm((got - want).reshape(n, -1), axis=1) / np.linalg.norm(want.reshape(n, -1), axis=1))
     assert worst < 10 * TOL_APPLY["f32"], worst
-    del out, U
+    del out
+    # ---- the Schur operator and its adjoint at sampled EVEN sites against the definition (Table V):
+    # the Ls = 24 tile kernel with the fused closed-form M_oo^-1 and > 2^31 element offsets versus generic elimination on the host
+    d.set_workspace(1, half_fields=1)
+    hb = d.field_bytes(1, half=True) // 4
+    ev = _sample_sites(L4, 8600, 5)
+    ev = ev[ev.sum(axis=1) % 2 == 0]
+    assert len(ev) >= 4096
+    ste = torch.from_numpy(ev).to(dev)
+    nb2 = _gather_two_hop(L4, psi, U, ste)
+    w = d.field(1, half=True)
+    for op, dag in ((DWF_SCHUR_EO, False), (DWF_SCHUR_EO | DWF_DAGGER, True)):
+        d.apply(op, x[:hb], w, 1)
+        can = d.export(w, 1, parity=0)
+        got = can[0][:, ste[:, 3], ste[:, 2], ste[:, 1], ste[:, 0]].permute(1, 0, 2, 3).cpu().numpy().astype(np.complex128)
+        del can
+        want = oracle.mpc_sites(L4, LS4, M5, MASS4, ev.astype(np.int32), *nb2, dagger=dag)
+        err = np.linalg.norm((got - want).ravel()) / np.linalg.norm(want.ravel())
+        assert err < TOL_APPLY["f32"], (dag, err)
+        worst = np.max(np.linalg.norm((got - want).reshape(len(ev), -1), axis=1) / np.linalg.norm(want.reshape(len(ev), -1), axis=1))
+        assert worst < 10 * TOL_APPLY["f32"], (dag, worst)
+    del w, nb2
     # ---- hermiticity at full size (oracle-free): <a, H b> = <H a, b>
     b2 = torch.roll(x, 12345)
     Ha, Hb = d.field(1), d.field(1)
@@ -151,8 +199,23 @@ def test_config4_ddw_sampled_and_cg_invariants(oracle):
     xs = d.field(1, half=True, zero=True)
     hist = np.array(d.cg_schur(b, xs, 100))
     assert np.all(np.diff(np.log(hist)) < 0.7) and hist[100] < hist[0]
-    w, q = d.field(1, half=True), d.field(1, half=True)
-    d.apply(DWF_SCHUR_EO, xs, w, 1); d.apply(DWF_SCHUR_EO | DWF_DAGGER, w, q, 1)
+    # true residual through the UNFUSED operator path (generic M_oo^-1 kernel, separate launches) on a second handle
+    import os
+    os.environ["DWF_NO_FUSE_MOOINV"] = "1"; os.environ["DWF_NO_FUSE_NORM"] = "1"
+    try:
+        d2 = Dwf(L4, LS4, M5, MASS4, DWF_F32)
+    finally:
+        del os.environ["DWF_NO_FUSE_MOOINV"], os.environ["DWF_NO_FUSE_NORM"]
+    d2.set_gauge(U)
+    del U
+    d.set_workspace(1, half_fields=0)                               # hand the CG workspace back before the second handle takes its own
+    d._ws = None
+    d2.set_workspace(1, half_fields=1)
+    w, q = d2.field(1, half=True), d2.field(1, half=True)
+    l0 = d2.launch_count()
+    d2.apply(DWF_SCHUR_EO, xs, w, 1)
+    assert d2.launch_count() - l0 == 3                               # K1, M_oo^-1, K2: the unfused form
+    d2.apply(DWF_SCHUR_EO | DWF_DAGGER, w, q, 1)
     rtrue = b - q
     r2 = d.norm2(rtrue, 1, half=True)[0]
     assert abs(r2 - hist[100]) / hist[100] < 1e-3, (r2, hist[100])

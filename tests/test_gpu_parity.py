@@ -221,7 +221,10 @@ def test_solve_red_black(oracle, prec, tol):
     iters, relres = rig.d.solve(en, psi, tol, 2000)
     psi_or, it_or = oracle.solve_rb(rig.U, eta, M5, mass, tol, 2000)
     got = rig.canonical(psi, 1)
-    assert iters < 2000 and abs(iters - it_or) <= 10                   # same stopping rule; the test sits every 10 iterations
+    # R25: the oracle stops at the first iteration below tol (tested every iteration), the driver tests every 10
+    # iterations: its count is the oracle's rounded up to a multiple of 10 (+- one test period for rounding drift in r_k)
+    assert iters < 2000 and iters % 10 == 0
+    assert -10 < iters - 10 * ((it_or + 9) // 10) <= 10, (iters, it_or)
     assert relres < 30 * tol                                           # true residual of the original system
     assert rel_l2(oracle.ddw(rig.U, got, M5, mass), eta) < 30 * tol    # ... and the oracle's operator agrees
     assert rel_l2(got, psi_or) < 100 * tol

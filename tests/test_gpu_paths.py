@@ -46,8 +46,11 @@ def test_fused_mooinv_vs_separate(monkeypatch, prec):
     rig = Rig(L, Ls, prec, mass, seed_U=41, ws_nrhs=nrhs)
     pe = gen.keep_parity(rig.spinor(nrhs, 42), L, 0)
     fused = [rig.apply(DWF_SCHUR_EO, pe, half=True), rig.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True)]
-    monkeypatch.setenv("DWF_NO_FUSE_MOOINV", "1")
-    sep = [rig.apply(DWF_SCHUR_EO, pe, half=True), rig.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True)]
+    monkeypatch.setenv("DWF_NO_FUSE_MOOINV", "1")                     # read at dwf_create: a second handle takes the unfused path
+    rig2 = Rig(L, Ls, prec, mass, seed_U=41, ws_nrhs=nrhs)
+    l0 = rig2.d.launch_count()
+    sep = [rig2.apply(DWF_SCHUR_EO, pe, half=True), rig2.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True)]
+    assert rig2.d.launch_count() - l0 == 2 * (1 + (nrhs + 1 + nrhs) + 1)   # import, K1 (one launch per rhs) + M_oo^-1 + K2, export
     for a, b in zip(fused, sep):
         assert np.array_equal(a, b)                   # same arithmetic in the same order: bit identical
 
@@ -58,9 +61,10 @@ def test_cg_graph_vs_stream(monkeypatch):
     b = rig.native(gen.keep_parity(rig.spinor(1, 2001), L, 0), 0)
     x1 = rig.d.field(1, half=True, zero=True)
     h1 = rig.d.cg_schur(b, x1, 20)
-    monkeypatch.setenv("DWF_CG_GRAPH", "1")
-    x2 = rig.d.field(1, half=True, zero=True)
-    h2 = rig.d.cg_schur(b, x2, 20)
+    monkeypatch.setenv("DWF_CG_GRAPH", "1")                           # read at dwf_create
+    rig2 = Rig(L, Ls, "f32", mass, seed_U=1001, ws_nrhs=1)
+    x2 = rig2.d.field(1, half=True, zero=True)
+    h2 = rig2.d.cg_schur(b, x2, 20)
     assert h1 == h2 and bool((x1 == x2).all())        # deterministic reductions: bit identical
 
 

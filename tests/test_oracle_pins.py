@@ -271,3 +271,43 @@ def test_site_list_mode(oracle):
     full = oracle.ddw(U, psi, M5, MASS)[0]
     want = np.stack([full[:, t, z, y, x] for (x, y, z, t) in sites])
     assert rel(got, want) < 1e-15
+
+
+def _gather2(L, U, psi_e, sites):
+    """Two-hop neighbourhoods in the layout oracle.mpc_sites expects (harness code: indexing only)."""
+    n, Ls = len(sites), psi_e.shape[1]
+    self_ = np.zeros((n, Ls, 4, 3), dtype=complex); nbr2 = np.zeros((n, 8, 8, Ls, 4, 3), dtype=complex)
+    links1 = np.zeros((n, 8, 3, 3), dtype=complex); links2 = np.zeros((n, 8, 8, 3, 3), dtype=complex)
+
+    def step(c, mu, d):
+        m = list(c); m[mu] = (m[mu] + d) % L[mu]
+        return m
+    for i, c in enumerate(sites):
+        self_[i] = psi_e[0, :, c[3], c[2], c[1], c[0]]
+        for mu in range(4):
+            for j, d in enumerate((+1, -1)):
+                y = step(c, mu, d)
+                src = c if d > 0 else y
+                links1[i, 2 * mu + j] = U[mu, src[3], src[2], src[1], src[0]]
+                for nu in range(4):
+                    for k, e in enumerate((+1, -1)):
+                        zc = step(y, nu, e)
+                        nbr2[i, 2 * mu + j, 2 * nu + k] = psi_e[0, :, zc[3], zc[2], zc[1], zc[0]]
+                        src2 = y if e > 0 else zc
+                        links2[i, 2 * mu + j, 2 * nu + k] = U[nu, src2[3], src2[2], src2[1], src2[0]]
+    return self_, nbr2, links1, links2
+
+
+@pytest.mark.parametrize("L,Ls", [((4, 4, 4, 4), 8), ((4, 6, 4, 8), 4)])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_mpc_site_list_mode(oracle, L, Ls, dagger):
+    """mpc_sites (configs[4] parity) equals the pinned full-volume M_pc (dense Schur complement pin,
+    test_oracle_dense.py) at EVERY even site, seam and corners included; a mass large enough to make the wall terms count."""
+    mass = 0.3
+    sites = [(x, y, z, t) for t in range(L[3]) for z in range(L[2]) for y in range(L[1]) for x in range(L[0]) if (x + y + z + t) % 2 == 0]
+    U = gen.gauge_random(L, 1000)
+    psi_e = gen.keep_parity(gen.spinor_gaussian(L, Ls, 1, 2000), L, 0)
+    got = oracle.mpc_sites(L, Ls, M5, mass, np.array(sites, dtype=np.int32), *_gather2(L, U, psi_e, sites), dagger=dagger)
+    full = oracle.mpc(U, psi_e, M5, mass, dagger=dagger)[0]
+    want = np.stack([full[:, t, z, y, x] for (x, y, z, t) in sites])
+    assert rel(got, want) < 1e-14
