@@ -35,9 +35,9 @@ FLOP_PER_SITE = 1320.0
 CHEB_ORDER, CHEB_NVEC, CHEB_LO, CHEB_HI = 64, 24, 0.01, 70.0
 CG_ITERS = 20
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (ncu --set full; average of the two
-# epilogue variants), filled in from the capture summarised in NCU_TRAFFIC_SOURCE
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 625.3e6
-NCU_TRAFFIC_SOURCE = "profiles/r1_10_cheb_tile.md"
+# epilogue variants): parsed from the ncu summary below (lines "traffic_bytes_per_launch: ..." and "commit: ..."), so that
+# the number always names the capture and the commit it was taken at
+NCU_TRAFFIC_SOURCE = "profiles/r2_cheb_traffic.md"
 WORKLOAD = "16^3x32xLs16 fp32: D_hop/D_DW/H_DW/D_PV (nrhs 1,12,48) + Schur(4) + BLAS-1 + order-64 Chebyshev(24) + 20 rb-CG it"
 
 
@@ -46,6 +46,24 @@ def peaks():
     if os.path.exists(p):
         return json.load(open(p)).get("hbm_gbs", 6650.0), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic():
+    """(bytes per launch or None, source string) from NCU_TRAFFIC_SOURCE."""
+    import re
+    path = os.path.join(ROOT, NCU_TRAFFIC_SOURCE)
+    try:
+        text = open(path).read()
+        val = float(re.search(r"^traffic_bytes_per_launch:\s*([0-9.eE+]+)", text, re.M).group(1))
+        commit = re.search(r"^commit:\s*(\S+)", text, re.M).group(1)
+        return val, f"{NCU_TRAFFIC_SOURCE} (ncu --set full at commit {commit})"
+    except Exception:
+        return None, f"{NCU_TRAFFIC_SOURCE} missing or unreadable"
+
+
+def schur_bytes(nrhs: int, v5: int, ls: int, real: int = 4) -> float:
+    """Algorithmic bytes of one M_pc apply: 120R + 288R/(Ls nrhs) per EVEN 5D site per rhs."""
+    return (v5 // 2) * nrhs * (120.0 * real + 288.0 * real / (ls * nrhs))
 
 
 def apply_bytes(nrhs: int, real: int = 4) -> float:
@@ -119,6 +137,68 @@ def oracle_sample(steps: int):
         psi = out / np.sqrt(np.mean(np.abs(out) ** 2))
     cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
     return times, cores
+
+
+def oracle_leg(name: str):
+    """One D.5 leg of the oracle, run in this (sub)process under whatever OMP_NUM_THREADS it was started with.  Prints a JSON line."""
+    import numpy as np
+    import dwf_inputs as gen
+    from oracle import dwf_oracle as oracle
+    oracle.build()
+    threads = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    if name == "ddw":                                        # (i) one fp64 D_DW apply, nrhs = 1, full 16^3x32x16 volume
+        U = gen.gauge_random(L, 1002); psi = gen.spinor_gaussian(L, LS, 1, 2002)
+        oracle.ddw(U, psi[:, :2], M5, MASS)
+        n = 3 if threads > 1 else 1
+        t0 = time.perf_counter()
+        for _ in range(n):
+            oracle.ddw(U, psi, M5, MASS)
+        dt = (time.perf_counter() - t0) / n
+        out = {"leg": "ddw", "threads": threads, "s_per_apply": round(dt, 3), "GFlop/s": round(FLOP_PER_SITE * V5 / dt / 1e9, 3),
+               "sample": f"{n} fp64 D_DW applies, nrhs=1, full 16^3x32x16 volume"}
+    elif name == "chebyshev":                                # (ii) Chebyshev of H_DW^2 on ONE vector of the 16^3x32x16 volume
+        order = CHEB_ORDER if threads > 1 else 2             # 2*order applies; the single-thread leg is a bounded sample, scaled
+        U = gen.gauge_random(L, 1002); psi = gen.spinor_gaussian(L, LS, 1, 2003)
+        oracle.ddw(U, psi[:, :2], M5, MASS)
+        t0 = time.perf_counter()
+        oracle.chebyshev(U, psi, M5, MASS, order, CHEB_LO, CHEB_HI)
+        dt = time.perf_counter() - t0
+        per_vec = dt * CHEB_ORDER / order
+        out = {"leg": "chebyshev", "threads": threads, "order_run": order, "s": round(dt, 2),
+               "s_per_order64_vector": round(per_vec, 2), "vectors/s": round(1.0 / per_vec, 5),
+               "sample": f"order-{order} filter of 1 vector (2x{order} operator applies), full 16^3x32x16 volume"
+                         + ("" if order == CHEB_ORDER else f", scaled x{CHEB_ORDER // order} to order {CHEB_ORDER}")}
+    elif name == "cg":                                       # (iii) 10 red-black CG iterations at configs[1] (8^4 x 16)
+        L8 = (8, 8, 8, 8)
+        U = gen.gauge_random(L8, 1001)
+        b = gen.keep_parity(gen.spinor_gaussian(L8, LS, 1, 2001), L8, 0)
+        oracle.cg_schur(U, b, M5, MASS, 1)
+        t0 = time.perf_counter()
+        oracle.cg_schur(U, b, M5, MASS, 10)
+        dt = time.perf_counter() - t0
+        out = {"leg": "cg", "threads": threads, "s": round(dt, 3), "iterations/s": round(11 / dt, 3),
+               "sample": "10 rb-CG iterations (+ the initial residual), 8^4x16, fp64"}
+    else:
+        raise SystemExit(f"unknown oracle leg {name}")
+    print(json.dumps(out), flush=True)
+
+
+def oracle_legs():
+    """the oracle, as it stands, on the host cores: legs (i) D_DW apply, (ii) order-64 Chebyshev on 1 vector,
+    (iii) 10 CG iterations at configs[1], each at OMP_NUM_THREADS = 1 and = nproc (subprocesses: OpenMP reads it at start-up)."""
+    res = {}
+    nproc = os.cpu_count() or 1
+    for leg in ("ddw", "chebyshev", "cg"):
+        for threads in (nproc, 1):
+            env = dict(os.environ, OMP_NUM_THREADS=str(threads))
+            try:
+                p = subprocess.run([sys.executable, os.path.abspath(__file__), "--oracle-leg", leg], env=env, capture_output=True,
+                                   text=True, timeout=600)
+                line = [ln for ln in p.stdout.splitlines() if ln.startswith("{")][-1]
+                res[f"{leg}_threads{threads}"] = json.loads(line)
+            except Exception as exc:                          # a leg that fails must not take the bench line with it
+                res[f"{leg}_threads{threads}"] = {"error": repr(exc)[:200]}
+    return res
 
 
 def run_reference(args):
@@ -302,6 +382,106 @@ def run_only_config4(args, dev):
     print(json.dumps(out), flush=True)
 
 
+def time_calls(fn, n, warm=3):
+    """Average milliseconds of fn(j) over n back-to-back calls (CUDA events on the current stream)."""
+    import torch
+    for j in range(warm):
+        fn(j)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for j in range(n):
+        fn(j)
+    b.record(); torch.cuda.synchronize()
+    return a.elapsed_time(b) / n
+
+
+def run_extras(dev, peak):
+    """Numbers of BASELINE.md that are not part of the timed fp32 step (SURVEY 8(d) D.1 rows [1], [2] fp64, [4]): run once,
+    after the step's buffers are freed.  Returns a dict for `detail`."""
+    import gc
+    import torch
+    import dwf_inputs as gen
+    from paper_2103_05034_b200 import DWF_DDW, DWF_F32, DWF_F64, DWF_HDW, DWF_SCHUR_EO, Dwf
+    out = {}
+    # ---- configs[2] in fp64 (the paper's own precision, PAPER.md L326): D_DW and H_DW at nrhs 1 / 12 / 48
+    d = Dwf(L, LS, M5, MASS, DWF_F64, device=dev)
+    d.set_gauge(torch.from_numpy(gen.gauge_random(L, 1002)).to(torch.complex128).to(dev))
+    g = torch.Generator(device=dev); g.manual_seed(2002)
+    for nrhs, reps in ((1, 20), (12, 3), (48, 2)):
+        nb = 4 if nrhs == 1 else 1
+        xs = [d.field(nrhs).normal_(generator=g) for _ in range(nb)]
+        ys = [d.field(nrhs) for _ in range(nb)]
+        for name, op in (("ddw", DWF_DDW), ("hdw", DWF_HDW)):
+            ms = time_calls(lambda j: d.apply(op, xs[j % nb], ys[j % nb], nrhs), reps, warm=2)
+            by = apply_bytes(nrhs, 8)
+            out[f"{name}_nrhs{nrhs}_fp64"] = {"ms": round(ms, 4), "GB/s": round(by / ms / 1e6, 1), "GFlop/s": round(FLOP_PER_SITE * V5 * nrhs / ms / 1e6, 1),
+                                             "frac_of_hbm_peak": round(by / ms / 1e6 / peak, 4)}
+        del xs, ys
+    d.set_workspace(4, half_fields=1)
+    xs4 = d.field(4, half=True).normal_(generator=g); ys4 = d.field(4, half=True)
+    ms = time_calls(lambda j: d.apply(DWF_SCHUR_EO, xs4, ys4, 4), 5)
+    by = schur_bytes(4, V5, LS, 8)
+    out["schur_nrhs4_fp64"] = {"ms": round(ms, 4), "GB/s": round(by / ms / 1e6, 1), "frac_of_hbm_peak": round(by / ms / 1e6 / peak, 4)}
+    del xs4, ys4
+    d.close(); del d
+    gc.collect(); torch.cuda.empty_cache()
+    # ---- configs[1]: 8^4 x 16, 50 rb-CG iterations (launch-bound size), fp32 and fp64
+    L8 = (8, 8, 8, 8)
+    for prec, code, cdt in (("fp32", DWF_F32, torch.complex64), ("fp64", DWF_F64, torch.complex128)):
+        d = Dwf(L8, LS, M5, MASS, code, device=dev)
+        d.set_gauge(torch.from_numpy(gen.gauge_random(L8, 1001)).to(cdt).to(dev))
+        d.set_workspace(1, half_fields=5)
+        g = torch.Generator(device=dev); g.manual_seed(2001)
+        b = d.field(1, half=True).normal_(generator=g); x = d.field(1, half=True, zero=True)
+
+        def cg50(j):
+            x.zero_(); d.cg_schur(b, x, 50)
+        for _ in range(3):
+            cg50(0)
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        for j in range(10):
+            cg50(j)
+        torch.cuda.synchronize()
+        ms = (time.perf_counter() - t0) * 1e3 / 10             # host clock: the call synchronises and is launch-bound
+        out[f"rb_cg_8^4x16_{prec}"] = {"iters": 50, "ms": round(ms, 3), "iterations/s": round(51 / ms * 1e3, 1)}
+        d.close(); del d, b, x
+    gc.collect(); torch.cuda.empty_cache()
+    # ---- configs[4]: 48^3 x 96 x 24 fp32, m = 0.00078: one D_DW apply, the Schur operator, 100 rb-CG iterations
+    free, _ = torch.cuda.mem_get_info()
+    if free < 120e9:
+        out["config4"] = {"skipped": f"needs ~110 GB of device memory, {free / 1e9:.0f} GB free"}
+        return out
+    L4, LS4, MASS4 = (48, 48, 48, 96), 24, 0.00078
+    v5 = L4[0] * L4[1] * L4[2] * L4[3] * LS4
+    d = Dwf(L4, LS4, M5, MASS4, DWF_F32, device=dev)
+    d.set_gauge(gen.gauge_random_torch(L4, 1004, dev, torch.complex64))
+    g = torch.Generator(device=dev); g.manual_seed(2004)
+    x, y = d.field(1).normal_(generator=g), d.field(1)
+    ms = time_calls(lambda j: d.apply(DWF_DDW, x, y, 1), 5, warm=2)
+    by = v5 * (48.0 * 4 + 72.0 * 4 / LS4)
+    out["ddw_48^3x96x24_fp32"] = {"ms": round(ms, 3), "GB/s": round(by / ms / 1e6, 1), "GFlop/s": round(FLOP_PER_SITE * v5 / ms / 1e6, 1),
+                                  "frac_of_hbm_peak": round(by / ms / 1e6 / peak, 4)}
+    del y
+    d.set_workspace(1, half_fields=5)
+    hb = d.field_bytes(1, half=True) // 4
+    bb = x[:hb].clone(); del x
+    xx = d.field(1, half=True, zero=True)
+    ms = time_calls(lambda j: d.apply(DWF_SCHUR_EO, bb, xx, 1), 3, warm=1)
+    by = schur_bytes(1, v5, LS4, 4)
+    out["schur_48^3x96x24_fp32"] = {"ms": round(ms, 3), "GB/s": round(by / ms / 1e6, 1), "frac_of_hbm_peak": round(by / ms / 1e6 / peak, 4)}
+    d.cg_schur(bb, xx, 2)
+    xx.zero_(); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(); hist = d.cg_schur(bb, xx, 100); b.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b)
+    out["rb_cg_48^3x96x24_fp32"] = {"iters": 100, "ms": round(ms, 1), "iterations/s": round(101 / ms * 1e3, 2),
+                                    "resid2_first_last": [hist[0], hist[-1]]}
+    d.close(); del d, bb, xx
+    gc.collect(); torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -312,7 +492,11 @@ def main():
     ap.add_argument("--only", default=None, help="time one part of the step only (for ncu captures), e.g. ddw_nrhs1, "
                     "hdw_nrhs1, dhop_nrhs1, ddw_nrhs12, ddw_nrhs48, schur_nrhs4, chebyshev, cg; prints a small JSON line")
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"], help="--only mode: precision")
+    ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / 8^4 / 48^3x96 legs of `detail` (run once, outside the timed step)")
+    ap.add_argument("--oracle-leg", default=None, help=argparse.SUPPRESS)
     args = ap.parse_args()
+    if args.oracle_leg:
+        return oracle_leg(args.oracle_leg)
     if args.impl == "reference":
         return run_reference(args)
 
@@ -442,8 +626,16 @@ def main():
                                           "GB/s": round(cheb_bytes(CHEB_ORDER, CHEB_NVEC) / t_cheb / 1e6, 1)}
     t_cg = avg_ms("cg")
     detail["rb_cg_16^3x32x16"] = {"ms": round(t_cg, 3), "iterations/s": round((CG_ITERS + 1) / t_cg * 1e3, 1)}
-    for name in ("a1_import_export", "schur_nrhs4", "blas1_nrhs12"):
-        detail[name] = {"ms": round(avg_ms(name), 4)}
+    detail["a1_import_export"] = {"ms": round(avg_ms("a1_import_export"), 4),
+                                  "GB/s": round(2 * 48.0 * 4 * V5 / avg_ms("a1_import_export") / 1e6, 1)}      # import + export: 2 x (R + W)
+    t_s = avg_ms("schur_nrhs4")
+    detail["schur_nrhs4"] = {"ms": round(t_s, 4), "GB/s": round(schur_bytes(4, V5, LS) / t_s / 1e6, 1),
+                             "frac_of_hbm_peak": round(schur_bytes(4, V5, LS) / t_s / 1e6 / peak, 4),
+                             "GFlop/s": round(FLOP_PER_SITE * V5 * 4 / t_s / 1e6, 1)}
+    t_b = avg_ms("blas1_nrhs12")
+    blas_bytes = (72.0 + 48.0 + 24.0) * 4 * V5 * 12                                   # axpy 72R + inner 48R + norm 24R per 5D site per rhs
+    detail["blas1_nrhs12"] = {"ms": round(t_b, 4), "GB/s": round(blas_bytes / t_b / 1e6, 1), "frac_of_hbm_peak": round(blas_bytes / t_b / 1e6 / peak, 4),
+                              "note": "axpy + inner + norm2 on 12 full fields, two host synchronisations inside"}
 
     # dominant kernel = dwf::hop_tile_kernel inside dwf_chebyshev (H_DW and H_DW + three-term-recurrence epilogues,
     # one launch per right-hand side and apply).  Its average launch duration = CUDA-event-bracketed call time
@@ -455,7 +647,7 @@ def main():
     ach = cheb_bytes(CHEB_ORDER, CHEB_NVEC) / t_cheb / 1e6
     roofline = {"bound": "hbm", "kernel": "dwf::hop_tile_kernel<float,16,32,...> (H_DW and H_DW+axpby epilogues, inside dwf_chebyshev)",
                 "achieved": round(ach, 1), "peak": peak, "peak_source": peak_src, "unit": "GB/s", "frac": round(ach / peak, 4),
-                "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "traffic_source": NCU_TRAFFIC_SOURCE,
+                "traffic": ncu_traffic()[0], "traffic_source": ncu_traffic()[1],
                 "algorithmic_bytes_per_launch": round(cheb_bytes(CHEB_ORDER, CHEB_NVEC) / n_launch),
                 "avg_launch_ms": round(t_cheb / n_launch, 4), "launches_per_call": n_launch,
                 "co_limit": "packed-fp32 FMA pipe: ~906 FFMA2/FADD2/FMUL2 per 2 5D sites, measured 100 lane-FMA/clk/SM (DESIGN.md sec. 5.2)",
@@ -476,7 +668,18 @@ def main():
                     "call": "dwf_apply_host(DWF_DDW, nrhs=1): pinned host canonical in -> H2D -> import -> D_DW -> export -> D2H",
                     "ms": round(e2e_s * 1e3, 3)},
             "roofline": roofline, "detail": detail}
+    if not args.no_extras and world == 1:
+        # free the step's buffers, then the legs that need their own handles (fp64, 8^4, 48^3 x 96)
+        del x1, y1, x12, y12, x48, y48, xs4, ys4, xc, yc, bcg, xcg, canon
+        d.close()
+        import gc
+        gc.collect(); torch.cuda.empty_cache()
+        try:
+            detail.update(run_extras(dev, peak))
+        except Exception as exc:                              # the headline line must survive a failing extra leg
+            detail["extras_error"] = repr(exc)[:300]
     if not args.no_cpu_baseline and world == 1:
+        line["cpu_baseline_legs"] = oracle_legs()
         times, cores = oracle_sample(5)
         tot = sum(times)
         line["cpu_baseline"] = {"value": round(FLOP_PER_SITE * V5 * len(times) / tot / 1e9, 3), "unit": "GFlop/s", "cores": cores,

@@ -14,6 +14,8 @@
 // global memory.  res = sigma * hop' + self with hop' built from the scaled links (sigma = 1 for
 // D_DW, H_DW, D_PV: no scaling pass).  The self term is computed first, while the copies land.
 #pragma once
+#include <type_traits>
+
 #include "dwf_aux.cuh"
 #include "dwf_hop.cuh"
 
@@ -246,36 +248,37 @@ hop_tile_kernel(const HopArgs<R> a) {
                 __syncthreads();
                 const R kappa = a.moo_kappa, v0scale = a.moo_v0scale, mass = a.mass;
                 G* obase_t = a.out[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS;   // the tile's blocks are one run
-                for (int row = threadIdx.x; row < TS * 12; row += TG::THREADS) {
+                // task = (row, real | imaginary part): TS*24 tasks = a whole number of passes of the CTA (3 for 32 sites x 256
+                // threads) with Ls values in registers each; the two tasks of a row sit in neighbouring lanes, so a pair reads
+                // and writes whole 16-byte groups
+                using H = typename std::conditional<VL == 2, float2, double>::type;        // one part of a group
+                const H* s_h = reinterpret_cast<const H*>(s_t);
+                for (int task = threadIdx.x; task < TS * 24; task += TG::THREADS) {
+                    const int row = task >> 1, part = task & 1;
                     const int c = row % 12;
                     const bool down = DAG ? (c >= 6) : (c < 6);
-                    R bre[LS], bim[LS];
+                    R b[LS];
 #pragma unroll
                     for (int kk = 0; kk < K; kk++) {
-                        const G g = s_t[row * (K + 1) + (down ? kk : K - 1 - kk)];
-                        if constexpr (VL == 2) {
-                            bre[2 * kk] = down ? g.x : g.y; bre[2 * kk + 1] = down ? g.y : g.x;
-                            bim[2 * kk] = down ? g.z : g.w; bim[2 * kk + 1] = down ? g.w : g.z;
-                        } else { bre[kk] = g.x; bim[kk] = g.y; }
+                        const H g = s_h[(row * (K + 1) + (down ? kk : K - 1 - kk)) * 2 + part];
+                        if constexpr (VL == 2) { b[2 * kk] = down ? g.x : g.y; b[2 * kk + 1] = down ? g.y : g.x; }
+                        else b[kk] = g;
                     }
-                    const R b0re = bre[0], b0im = bim[0];
-                    bre[0] = R(0); bim[0] = R(0);
+                    const R b0 = b[0];
+                    b[0] = R(0);
 #pragma unroll
-                    for (int j = 1; j < LS; j++) { bre[j] = kappa * (bre[j] + bre[j - 1]); bim[j] = kappa * (bim[j] + bim[j - 1]); }
-                    const R v0re = v0scale * (b0re - mass * bre[LS - 1]);
-                    const R v0im = v0scale * (b0im - mass * bim[LS - 1]);
+                    for (int j = 1; j < LS; j++) b[j] = kappa * (b[j] + b[j - 1]);
+                    const R v0 = v0scale * (b0 - mass * b[LS - 1]);
                     R pw = R(1);
 #pragma unroll
-                    for (int j = 0; j < LS; j++) { bre[j] = fma(pw, v0re, bre[j]); bim[j] = fma(pw, v0im, bim[j]); pw *= kappa; }
-                    G* orow = obase_t + (size_t)row * K;
+                    for (int j = 0; j < LS; j++) { b[j] = fma(pw, v0, b[j]); pw *= kappa; }
+                    H* orow = reinterpret_cast<H*>(obase_t + (size_t)row * K);
 #pragma unroll
                     for (int kk = 0; kk < K; kk++) {
-                        G g;
-                        if constexpr (VL == 2) {
-                            g.x = down ? bre[2 * kk] : bre[2 * kk + 1]; g.y = down ? bre[2 * kk + 1] : bre[2 * kk];
-                            g.z = down ? bim[2 * kk] : bim[2 * kk + 1]; g.w = down ? bim[2 * kk + 1] : bim[2 * kk];
-                        } else { g.x = bre[kk]; g.y = bim[kk]; }
-                        orow[down ? kk : K - 1 - kk] = g;
+                        H g;
+                        if constexpr (VL == 2) { g.x = down ? b[2 * kk] : b[2 * kk + 1]; g.y = down ? b[2 * kk + 1] : b[2 * kk]; }
+                        else g = b[kk];
+                        orow[(down ? kk : K - 1 - kk) * 2 + part] = g;
                     }
                 }
                 release_buffers();                             // the solver's reads of the buffer are complete (values consumed)
