@@ -38,6 +38,7 @@ struct dwf_ctx {
     void* ws; size_t ws_bytes;
     double* partial;      // reduction partials [blocks][nrhs][2]
     size_t partial_doubles;   // its size: covers blas_blocks(nrhs) * nrhs * 2 for every nrhs <= MAX_NRHS
+    unsigned* ticket;     // CTA completion counter of the fused norm (zero between launches)
     double* scal;         // device scalars (reduction results, CG history)
     double* scal_host;    // pinned mirror
     int sm_count, device;
@@ -196,6 +197,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
            && cudaMalloc((void**)&h->lex, lex.size() * sizeof(int)) == cudaSuccess
            && cudaMalloc((void**)&h->partial, h->partial_doubles * sizeof(double)) == cudaSuccess
            && cudaMalloc((void**)&h->scal, SCAL_DOUBLES * sizeof(double)) == cudaSuccess
+           && cudaMalloc((void**)&h->ticket, 64) == cudaSuccess && cudaMemset(h->ticket, 0, 64) == cudaSuccess
            && cudaMallocHost((void**)&h->scal_host, SCAL_DOUBLES * sizeof(double)) == cudaSuccess
            && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) == cudaSuccess;
     ok = ok && cudaMemcpy(h->nbr, nbr.data(), nbr.size() * sizeof(int), cudaMemcpyHostToDevice) == cudaSuccess
@@ -207,7 +209,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
 
 extern "C" int dwf_destroy(dwf_handle h) {
     if (!h) return DWF_EINVAL;
-    cudaFree(h->gauge); cudaFree(h->glinks); cudaFree(h->inv_lex); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal);
+    cudaFree(h->gauge); cudaFree(h->glinks); cudaFree(h->inv_lex); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal); cudaFree(h->ticket);
     if (h->scal_host) cudaFreeHost(h->scal_host);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     delete h;
@@ -299,7 +301,8 @@ extern "C" int dwf_export(dwf_handle h, const void* native, void* canonical, int
 // ------------------------------------------------------------------------------------------------
 // Stencil dispatch
 // ------------------------------------------------------------------------------------------------
-enum HopMode { HM_HOP, HM_HOP_SELF, HM_HOP_SELF_G5, HM_HOP_SELF_G5_AXPBY, HM_SELF, HM_HOP_MOOINV /* tiled only */ };
+enum HopMode { HM_HOP, HM_HOP_SELF, HM_HOP_SELF_G5, HM_HOP_SELF_G5_AXPBY, HM_SELF, HM_HOP_MOOINV /* tiled only */,
+               HM_HOP_SELF_AXPBY_NORM /* tiled only: CG residual update fused into the adjoint Schur K2 */ };
 
 struct HopCall {            // precision-independent description of one launch
     int mode; bool dag;
@@ -307,8 +310,9 @@ struct HopCall {            // precision-independent description of one launch
     const void* in_hop[2]; const void* in_self[2]; void* out[2]; const void* y[2]; const void* z[2];
     double c_hop, mass, ax_a, ax_b, ax_c;
     int nrhs;
-    double* norm_partial;   // tiled HM_HOP_SELF only: also write |out|^2 partials [item][warp][2] (nrhs = 1)
-    long long* norm_count;  // ... and return how many partials there are
+    double* norm_out;       // tiled HM_HOP_SELF (not dag) and HM_HOP_SELF_AXPBY_NORM, nrhs = 1: also *norm_out = |out|^2 (device), summed
+                            // inside the launch (dwf_tile.cuh NORM epilogue)
+    const double* ax_num; const double* ax_den;   // HM_HOP_SELF_AXPBY_NORM: ax_a = -(*ax_num / *ax_den), read on the device
 };
 
 // Is the tiled persistent stencil (dwf_tile.cuh) instantiated for this handle?  Lattice made of whole tiles, Ls 16 (16- or
@@ -349,7 +353,8 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.glinks[0] = (const R*)h->glinks;
     a.glinks[1] = (const R*)((const char*)h->glinks + (size_t)h->V4h * lsite);
     a.sigma = (R)(-2.0 * k.c_hop);                                             // links carry the factor -1/2
-    a.norm_partial = k.norm_partial;
+    a.norm_partial = h->partial; a.norm_out = k.norm_out; a.ticket = h->ticket;
+    a.ax_num = k.ax_num; a.ax_den = k.ax_den;
     {
         const double kappa = 1.0 / (5.0 - h->M5);
         a.moo_kappa = (R)kappa; a.moo_v0scale = (R)(kappa / (1.0 + k.mass * std::pow(kappa, (double)h->Ls)));
@@ -359,7 +364,6 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
 #define TILEK(LS, TSV, DAG, SELF, G5, AX, MOO, NRM) do { \
         using TG = TileGeom<R, LS, TSV>; \
         auto kern = hop_tile_kernel<R, LS, TSV, DAG, true, SELF, G5, AX, MOO, NRM>; \
-        if (NRM && k.norm_count) *k.norm_count = a.nitems * (TG::THREADS / 32); \
         static unsigned long long attr_done = 0;              /* per kernel instantiation: devices whose attribute is set */ \
         if (!((attr_done >> (h->device & 63)) & 1ull)) { \
             cudaError_t e_ = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TG::SMEM_BYTES); \
@@ -382,12 +386,14 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
         case HM_HOP:               if (k.dag) TILEK(LS, TSV, true, false, false, false, false, false); else TILEK(LS, TSV, false, false, false, false, false, false); break; \
         case HM_HOP_MOOINV:        if (k.dag) TILEK(LS, TSV, true, false, false, false, true, false); else TILEK(LS, TSV, false, false, false, false, true, false); break; \
         case HM_HOP_SELF:          if (k.dag) TILEK(LS, TSV, true, true, false, false, false, false); \
-                                   else if (k.norm_partial) TILEK(LS, TSV, false, true, false, false, false, true); \
+                                   else if (k.norm_out) TILEK(LS, TSV, false, true, false, false, false, true); \
                                    else TILEK(LS, TSV, false, true, false, false, false, false); break; \
         case HM_HOP_SELF_G5:       TILEK(LS, TSV, false, true, true, false, false, false); break; \
         case HM_HOP_SELF_G5_AXPBY: TILEK(LS, TSV, false, true, true, true, false, false); break; \
+        case HM_HOP_SELF_AXPBY_NORM: TILEK(LS, TSV, true, true, false, true, false, true); break; \
         default: FAIL(h, DWF_EINVAL, "bad hop mode"); \
     }
+    if ((k.norm_out || k.mode == HM_HOP_SELF_AXPBY_NORM) && (!TS || k.nrhs != 1)) FAIL(h, DWF_EINVAL, "fused norm needs the tiled kernel and nrhs = 1");
     // Right-hand sides are processed in chunks (one launch each) so that the working set of a chunk keeps
     // the L2 reuse of the single-rhs case; CTAs of one chunk run tile-major, rhs-minor.
     const int RC = h->rhs_chunk;
@@ -454,7 +460,16 @@ static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, co
 // out = M_ee in - 1/4 Dhop_eo tmp_o     [M_eo = M_oe = -1/2 Dhop].  dag: every factor adjoint.
 // norm_out != NULL (nrhs = 1, not dag): also *norm_out = |out|^2 on the device; fused into K2 when the tiled kernel applies.
 static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nrhs, int half, double* dev_out, int ostride, int ncomp);
-static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs, double* norm_out = nullptr) {
+// Can the |out|^2 of a stencil launch be summed inside the launch (tiled kernel, one rhs, partials fit the scratch)?
+static bool norm_fusable(const dwf_ctx* h, int nrhs) {
+    return tiled_ok(h) && !h->no_fuse_moo && !h->no_fuse_norm && nrhs == 1
+        && (size_t)h->sm_count * 4 * 32 * 2 <= h->partial_doubles;              // <= 4 CTAs per SM, <= 32 warps per CTA
+}
+struct SchurFuse {          // dag only (CG, q = M^dag w): r <- r - (num/den) q instead of storing q, and *norm_out = |r|^2
+    void* r; const double* num; const double* den;
+};
+static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, int nrhs, double* norm_out = nullptr,
+                    const SchurFuse* fuse = nullptr) {
     // K1: tmp_o = M_oo^-1 Dhop_oe in -- one launch when the tiled kernel applies (M_oo^-1 fused as its epilogue)
     const bool fused = tiled_ok(h) && !h->no_fuse_moo;
     HopCall k1{};
@@ -465,18 +480,16 @@ static int schur_op(dwf_ctx* h, bool dag, const void* in, void* out, void* tmp, 
     HopCall k2{};
     k2.mode = HM_HOP_SELF; k2.dag = dag; k2.nslots = 1; k2.parity0 = 0; k2.nrhs = nrhs;
     k2.in_hop[0] = tmp; k2.in_self[0] = in; k2.out[0] = out; k2.c_hop = -0.25; k2.mass = h->mass;
-    long long nparts = 0;
-    const long long max_parts = (long long)(h->partial_doubles / 2);
-    const long long tile_warps = h->tile_sites ? (h->V4h / h->tile_sites) * ((long long)h->tile_sites * h->Ls / vl(h) / 32) : 0;
-    const bool fuse_norm = norm_out && fused && nrhs == 1 && !dag && tile_warps <= max_parts && !h->no_fuse_norm;
-    if (fuse_norm) { k2.norm_partial = h->partial; k2.norm_count = &nparts; }
-    if (int rc = launch_hop(h, k2)) return rc;
-    if (!norm_out) return DWF_OK;
-    if (fuse_norm && nparts > 0) {
-        reduce_final_kernel<<<1, 256, 0, h->stream>>>(h->partial, (int)nparts, 1, norm_out, 1, 1);
-        LAUNCH_CHECK(h);
-        return DWF_OK;
+    if (fuse) {                                               // out = r - alpha (M_pc^dag in), |out|^2: one launch, q never stored
+        if (!dag || !norm_out || !norm_fusable(h, nrhs)) FAIL(h, DWF_EINVAL, "fused residual update: adjoint Schur, tiled kernel, nrhs = 1");
+        k2.mode = HM_HOP_SELF_AXPBY_NORM; k2.out[0] = fuse->r; k2.z[0] = fuse->r; k2.y[0] = fuse->r;
+        k2.ax_a = 0.0; k2.ax_b = 0.0; k2.ax_c = 1.0; k2.ax_num = fuse->num; k2.ax_den = fuse->den; k2.norm_out = norm_out;
+        return launch_hop(h, k2);
     }
+    const bool fuse_norm = norm_out && !dag && norm_fusable(h, nrhs);
+    if (fuse_norm) k2.norm_out = norm_out;
+    if (int rc = launch_hop(h, k2)) return rc;
+    if (!norm_out || fuse_norm) return DWF_OK;
     return reduce_to(h, true, out, nullptr, nrhs, 1, norm_out, 1, 1);
 }
 
@@ -816,13 +829,23 @@ static int cg_t(dwf_ctx* h, const void* b, void* x, int iters, int nrhs = 1, dou
     if (int rc = op2(w, q, tmp)) return rc;
     cg_init_kernel<R><<<blocks, 256, 0, st>>>((const G*)b, q, r, p, ng, BS, nrhs, h->partial); LAUNCH_CHECK(h);
     reduce_final_kernel<<<nrhs, 256, 0, st>>>(h->partial, (int)blocks, nrhs, hist, 1, 1); LAUNCH_CHECK(h);
+    // Fused iteration (tiled kernel, one rhs, red-black): 5 launches, 15 half-vector passes instead of 8 launches and 19 passes:
+    //   w = M p with |w|^2 summed inside K2;  r <- r - alpha M^dag w with |r|^2 summed inside the adjoint K2 (q is never stored);
+    //   x += alpha p and p = r + beta p in one pass.
+    const bool fusedcg = kind == 0 && norm_fusable(h, nrhs);
     for (int k = 0; k < iters; k++) {
         double* hk = hist + (size_t)k * nrhs; double* hk1 = hk + nrhs; double* pk = pAp + (size_t)k * nrhs;
         if (int rc = op1(p, w, tmp, pk)) return rc;                                // w = O1 p and <p, A p> = |w|^2
-        if (int rc = op2(w, q, tmp)) return rc;
-        cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, BS, nrhs, hk, pk, h->partial); LAUNCH_CHECK(h);
-        reduce_final_kernel<<<nrhs, 256, 0, st>>>(h->partial, (int)blocks, nrhs, hk1, 1, 1); LAUNCH_CHECK(h);
-        cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, BS, nrhs, hk1, hk); LAUNCH_CHECK(h);
+        if (fusedcg) {
+            const SchurFuse f{r, hk, pk};
+            if (int rc = schur_op(h, true, w, nullptr, tmp, nrhs, hk1, &f)) return rc;
+            cg_update_xp_kernel<R><<<blocks, 256, 0, st>>>((G*)x, p, r, ng, BS, nrhs, hk, pk, hk1); LAUNCH_CHECK(h);
+        } else {
+            if (int rc = op2(w, q, tmp)) return rc;
+            cg_update_xr_kernel<R><<<blocks, 256, 0, st>>>((G*)x, r, p, q, ng, BS, nrhs, hk, pk, h->partial); LAUNCH_CHECK(h);
+            reduce_final_kernel<<<nrhs, 256, 0, st>>>(h->partial, (int)blocks, nrhs, hk1, 1, 1); LAUNCH_CHECK(h);
+            cg_update_p_kernel<R><<<blocks, 256, 0, st>>>(p, r, ng, BS, nrhs, hk1, hk); LAUNCH_CHECK(h);
+        }
         if (done) *done = k + 1;
         if (tol_rel > 0.0 && ((k + 1) % check_every == 0 || k + 1 == iters)) {      // stopping test (nrhs = 1): |r_k|^2 <= tol^2 |r_0|^2
             CUDA_TRY(h, cudaMemcpyAsync(h->scal_host, hist, sizeof(double), cudaMemcpyDeviceToHost, st));

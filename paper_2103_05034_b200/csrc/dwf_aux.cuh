@@ -318,6 +318,27 @@ cg_update_xr_kernel(typename Prec<R>::G* x, typename Prec<R>::G* r, const typena
     block_combine(sre, sim, rhs, nrhs, partial);
 }
 
+// fused iteration (dwf_api.cu cg_t): x += alpha p ; p = r + beta p   (r already updated by the adjoint Schur launch)
+template <typename R>
+__global__ void __launch_bounds__(256)
+cg_update_xp_kernel(typename Prec<R>::G* x, typename Prec<R>::G* p, const typename Prec<R>::G* __restrict__ r,
+                    long long ngroups, int BS, int nrhs, const double* __restrict__ rr_old, const double* __restrict__ pAp,
+                    const double* __restrict__ rr_new) {
+    using V = typename Prec<R>::V;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int rhs = (int)((e / BS) % nrhs);
+    const R alpha = pAp[rhs] != 0.0 ? (R)(rr_old[rhs] / pAp[rhs]) : R(0);
+    const R beta = rr_old[rhs] != 0.0 ? (R)(rr_new[rhs] / rr_old[rhs]) : R(0);
+    for (; e < ngroups; e += stride) {
+        const CV<V> rv = unpack(ldg_nc(r + e));
+        CV<V> pp = unpack(p[e]), xx = unpack(x[e]);
+        xx.re = vfma(alpha, pp.re, xx.re); xx.im = vfma(alpha, pp.im, xx.im);
+        pp.re = vfma(beta, pp.re, rv.re); pp.im = vfma(beta, pp.im, rv.im);
+        x[e] = pack(xx); p[e] = pack(pp);
+    }
+}
+
 template <typename R>
 __global__ void __launch_bounds__(256)
 cg_update_p_kernel(typename Prec<R>::G* p, const typename Prec<R>::G* __restrict__ r, long long ngroups, int BS, int nrhs,

@@ -43,7 +43,11 @@ template <typename R> struct HopArgs {
     R sigma;               // res = sigma * hop' + self  with hop' built from the (-1/2)-scaled links
     R moo_kappa, moo_v0scale;   // fused M_oo^-1 epilogue: 1/(5-M5), kappa / (1 + m kappa^Ls)
     long long nitems;      // work items (tile, rhs, parity slot) of this launch
-    double* norm_partial;  // NORM epilogue: |out|^2 partials [item][warp][2]
+    double* norm_partial;  // NORM epilogue: |out|^2 partials [CTA][warp][2] (each warp's running sum over its items, in item order)
+    double* norm_out;      // ... summed in (CTA, warp) order by the last CTA to finish and written here
+    unsigned* ticket;      // ... CTA completion counter (zero on entry, reset to zero by the last CTA)
+    const double* ax_num;  // AXPBY with a device scalar: if non-NULL, ax_a = -(*ax_num / *ax_den) (0 when *ax_den == 0):
+    const double* ax_den;  //   the CG residual update r <- r - alpha q fused into the launch that produces q
     long long ngroups;     // ceil(V4h / G)
     long long chunk_groups;
     R c_hop, c_diag, mass;

@@ -170,6 +170,11 @@ hop_tile_kernel(const HopArgs<R> a) {
     const int ls = threadIdx.x / K;                            // site within the tile
     const int k = threadIdx.x - ls * K;
 
+    double norm_run = 0.0;                                     // NORM: this warp's running |out|^2 (lane 0), items in launch order
+    R ax_a = a.ax_a;
+    if constexpr (AXPBY) {
+        if (a.ax_num) { const double den = *a.ax_den; ax_a = den != 0.0 ? (R)(-(*a.ax_num / den)) : R(0); }
+    }
     for (int it = 0; w < a.nitems; it++, w += gridDim.x) {
         long long gg; int r, pi;
         decode(w, gg, r, pi);
@@ -299,27 +304,60 @@ hop_tile_kernel(const HopArgs<R> a) {
             const G* y = a.y[pi] + obase;
             const G* z = a.z[pi] + obase;
 #pragma unroll
-            for (int c = 0; c < 12; c++) {
-                const CV<V> yy = unpack(ldg_nc(y + c * K));
-                const CV<V> zz = unpack(ld_plain(z + c * K));
-                acc[c].re = vfma(a.ax_c, zz.re, vfma(a.ax_b, yy.re, vmul(a.ax_a, acc[c].re)));
-                acc[c].im = vfma(a.ax_c, zz.im, vfma(a.ax_b, yy.im, vmul(a.ax_a, acc[c].im)));
+            for (int c = 0; c < 12; c++) { acc[c].re = vmul(ax_a, acc[c].re); acc[c].im = vmul(ax_a, acc[c].im); }
+            if (a.ax_b != R(0)) {                              // a zero coefficient means "operand absent": it is not read
+#pragma unroll
+                for (int c = 0; c < 12; c++) {
+                    const CV<V> yy = unpack(ldg_nc(y + c * K));
+                    acc[c].re = vfma(a.ax_b, yy.re, acc[c].re); acc[c].im = vfma(a.ax_b, yy.im, acc[c].im);
+                }
+            }
+            if (a.ax_c != R(0)) {
+#pragma unroll
+                for (int c = 0; c < 12; c++) {
+                    const CV<V> zz = unpack(ld_plain(z + c * K));
+                    acc[c].re = vfma(a.ax_c, zz.re, acc[c].re); acc[c].im = vfma(a.ax_c, zz.im, acc[c].im);
+                }
             }
         }
         G* o = a.out[pi] + obase;
 #pragma unroll
         for (int c = 0; c < 12; c++) __stcs(o + c * K, pack(acc[c]));          // streaming store: the output is not re-read by this launch
         if constexpr (NORM) {
-            // |out|^2 of this item, fp64: fixed shuffle tree inside the warp, one partial per (item, warp) at a fixed slot,
-            // summed later in slot order by reduce_final_kernel: deterministic whichever CTA ran the item.
+            // |out|^2 of this item, fp64: fixed shuffle tree inside the warp, added to the warp's running sum.  The items of a
+            // CTA are a fixed function of the launch geometry, so the result does not depend on the timing of the CTAs.
             double sre = 0, sim = 0;
 #pragma unroll
             for (int c = 0; c < 12; c++) acc_inner(sre, sim, acc[c], acc[c]);
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) sre += __shfl_xor_sync(0xffffffffu, sre, off);
-            if ((threadIdx.x & 31) == 0) {
-                double* slot = a.norm_partial + ((size_t)w * NWARPS + (threadIdx.x >> 5)) * 2;
-                slot[0] = sre; slot[1] = 0.0;
+            norm_run += sre;
+        }
+    }
+    if constexpr (NORM) {
+        // one partial per (CTA, warp); the last CTA to arrive sums them in (CTA, warp) order: deterministic, no extra launch
+        __shared__ bool s_last;
+        if ((threadIdx.x & 31) == 0) {
+            double* slot = a.norm_partial + ((size_t)blockIdx.x * NWARPS + (threadIdx.x >> 5)) * 2;
+            slot[0] = norm_run; slot[1] = 0.0;
+        }
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1);
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            __shared__ double s_sum[TG::THREADS];
+            const int n = (int)(gridDim.x * NWARPS);
+            double t = 0;
+            for (int k = threadIdx.x; k < n; k += TG::THREADS) t += __ldcg(a.norm_partial + (size_t)k * 2);
+            s_sum[threadIdx.x] = t;
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                double tot = 0;
+                for (int k = 0; k < TG::THREADS; k++) tot += s_sum[k];
+                *a.norm_out = tot;
+                *a.ticket = 0u;
             }
         }
     }
