@@ -311,6 +311,15 @@ def run_only(args, dev):
         ms = (time.perf_counter() - t0) * 1e3 / args.steps
         print(json.dumps({"only": name, "prec": args.prec, "iters": 50, "ms": round(ms, 3), "iterations/s": round(51 / ms * 1e3, 1)}), flush=True)
         return
+    if name == "blas1":                                      # a7 on 12 full fields: axpy, inner, norm2
+        d = Dwf(L, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)
+        g = torch.Generator(device=dev); g.manual_seed(2002)
+        x, y = d.field(12).normal_(generator=g), d.field(12).normal_(generator=g)
+        ms = time_calls(lambda j: (d.axpy([0.5 + 0.1j] * 12, x, y, 12), d.inner(x, y, 12), d.norm2(x, 12)), args.steps)
+        by = 144.0 * (4 if f32 else 8) * V5 * 12
+        print(json.dumps({"only": name, "prec": args.prec, "nrhs": 12, "ms": round(ms, 4), "GB/s": round(by / ms / 1e6, 1),
+                          "frac_of_hbm_peak": round(by / ms / 1e6 / peaks()[0], 4)}), flush=True)
+        return
     d = Dwf(L, LS, M5, MASS, DWF_F32 if f32 else DWF_F64, device=dev)
     d.set_gauge(torch.from_numpy(gen.gauge_random(L, 1002)).to(d.cdtype).to(dev))
     g = torch.Generator(device=dev); g.manual_seed(2002)
@@ -490,7 +499,7 @@ def main():
     ap.add_argument("--impl", default="dwf", choices=["dwf", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--only", default=None, help="time one part of the step only (for ncu captures), e.g. ddw_nrhs1, "
-                    "hdw_nrhs1, dhop_nrhs1, ddw_nrhs12, ddw_nrhs48, schur_nrhs4, chebyshev, cg; prints a small JSON line")
+                    "hdw_nrhs1, dhop_nrhs1, ddw_nrhs12, ddw_nrhs48, schur_nrhs4, chebyshev, cg, cg_8, blas1, ddw_48, cg_48, subspace, solve; prints a small JSON line")
     ap.add_argument("--prec", default="f32", choices=["f32", "f64"], help="--only mode: precision")
     ap.add_argument("--no-extras", action="store_true", help="skip the fp64 / 8^4 / 48^3x96 legs of `detail` (run once, outside the timed step)")
     ap.add_argument("--oracle-leg", default=None, help=argparse.SUPPRESS)

@@ -63,7 +63,6 @@ template <typename R, int LS, int TS> struct TileGeom {
     static constexpr int K = LS / Prec<R>::VL;
     static constexpr int THREADS = TS * K;
     static constexpr int MIN_CTAS = THREADS <= 128 ? DWF_MINCTAS128 : THREADS <= 192 ? DWF_MINCTAS192 : THREADS <= 256 ? DWF_MINCTAS256 : 1;
-    static constexpr int NSTI = DWF_INT_STAGES;
     static constexpr int BS = 12 * K;
     static constexpr unsigned INTERIOR_BYTES = TS * BS * 16;
     static constexpr unsigned LINK_BYTES = TS * TileLinks<R>::SITE * sizeof(R);
@@ -72,6 +71,10 @@ template <typename R, int LS, int TS> struct TileGeom {
     // the fused M_oo^-1 epilogue transposes the tile through the interior buffer with rows padded by one group
     static constexpr unsigned TRANS_BYTES = TS * 12 * (K + 1) * 16;
     static constexpr unsigned INT_STRIDE = INTERIOR_BYTES > TRANS_BYTES ? INTERIOR_BYTES : TRANS_BYTES;
+    // Interior buffers: one.  With two CTAs per SM the refill of one CTA's buffer is covered by the other CTA; for the CTA that
+    // has the SM to itself (384 threads: fp32 Ls 24) a second buffer was measured SLOWER on B200 (48^3x96x24 D_DW 28.3 ms
+    // against 21.0 ms): the 72 KB it takes away from L1 cost more (halo and s+-1 loads hit L1) than the exposed refill.
+    static constexpr int NSTI = DWF_INT_STAGES;
     static constexpr unsigned SMEM_BYTES = 128 + NSTI * INT_STRIDE + 2 * SMALL_BYTES;
 };
 
@@ -113,7 +116,7 @@ __device__ __forceinline__ void tile_dir(CV<V> (&acc)[12], const G* psi, const i
 template <typename R, int LS, int TS, bool DAG, bool HOP, bool SELF, bool G5, bool AXPBY, bool MOO = false, bool NORM = false>
 __global__ void __launch_bounds__(TileGeom<R, LS, TS>::THREADS, TileGeom<R, LS, TS>::MIN_CTAS)
 hop_tile_kernel(const HopArgs<R> a) {
-    static_assert(!MOO || (HOP && !SELF && !G5 && !AXPBY && TileGeom<R, LS, TS>::NSTI == 1), "fused M_oo^-1 follows a bare hop");
+    static_assert(!MOO || (HOP && !SELF && !G5 && !AXPBY), "fused M_oo^-1 follows a bare hop");
     using V = typename Prec<R>::V;
     using G = typename Prec<R>::G;
     using TG = TileGeom<R, LS, TS>;
@@ -246,7 +249,7 @@ hop_tile_kernel(const HopArgs<R> a) {
                 // interior buffer (rows = (site, component), padded by one group against bank conflicts), then one
                 // thread per row walks s in registers and stores the row (contiguous in the output block).
                 constexpr int VL = Prec<R>::VL;
-                G* s_t = reinterpret_cast<G*>(smem + 128);
+                G* s_t = reinterpret_cast<G*>(smem + 128 + ib * TG::INT_STRIDE);    // this item's interior buffer
                 __syncthreads();                               // every warp is done reading the interior
 #pragma unroll
                 for (int c = 0; c < 12; c++) s_t[(ls * 12 + c) * (K + 1) + k] = pack(acc[c]);
