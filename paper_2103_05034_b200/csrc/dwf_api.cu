@@ -43,7 +43,10 @@ struct dwf_ctx {
     double* scal_host;    // pinned mirror
     int sm_count, device;
     bool no_fuse_moo, no_fuse_norm;   // DWF_NO_FUSE_MOOINV / DWF_NO_FUSE_NORM, read once at dwf_create (the unfused reference path)
-    int cg_graph;         // DWF_CG_GRAPH, read once at dwf_create
+    int cg_graph;         // DWF_CG_GRAPH, read once at dwf_create: 0 never, 1 always, unset (-1): launch-bound sizes only
+    // the instantiated CUDA graph of the last CG solve and the arguments it was captured for (re-launched when they recur)
+    long long cg_launches;
+    cudaGraphExec_t cg_exec; const void* cg_b; void* cg_x; void* cg_ws; size_t cg_ws_bytes; int cg_iters, cg_nrhs, cg_kind;
     long long blk_sites;  // sites per parity in one lattice block of the native site order
     int tile_sites;       // sites per parity in one tile of the native site order (0: lattice is not made of whole tiles)
     int sg_shift;         // block order [site group][rhs][site in group]: log2(group size)
@@ -112,13 +115,20 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     std::vector<int> idx_of(V4);                                                // lex site -> index within its parity
     long long cnt[2] = {0, 0};
     int nb[4], nt[4]; for (int i = 0; i < 4; i++) { nb[i] = L[i] / B[i]; nt[i] = B[i] / T[i]; }
-    // Order of the lattice blocks: DWF_BLOCK_ORDER=morton walks them along a Z-order curve (neighbouring blocks in all four
-    // directions stay close in the order: shorter reuse distance in L2), default = lexicographic (x fastest).
+    // Order of the lattice blocks: lexicographic (x fastest).  It re-reads the +-t halo of a block one 3-D slab of blocks later;
+    // when that slab no longer fits L2 the z and t halos come from DRAM twice (48^3 x 96 x 24: DRAM reads 2.15x the algorithmic
+    // bytes, ncu).  Two alternatives are kept behind DWF_BLOCK_ORDER for measurement and are NOT the default: "panel" (the (x,y,z)
+    // cross-section cut into panels of px x py x pz blocks whose slab fits DWF_L2_BUDGET_MB, t swept inside each panel) and "morton"
+    // (Z-order curve).  Measured on B200: panel 23.5 ms against 21.0 ms per D_DW apply at 48^3 x 96 x 24 (the kernel is bound by its
+    // LSU wavefronts there, 68 %, not by DRAM), +-1 % at 16^3 x 32 in either precision; morton +-2 %.
     std::vector<std::array<int, 4>> blocks;
     for (int bt = 0; bt < nb[3]; bt++) for (int bz = 0; bz < nb[2]; bz++) for (int by = 0; by < nb[1]; by++) for (int bx = 0; bx < nb[0]; bx++)
         blocks.push_back({bx, by, bz, bt});
     {
         const char* ord = getenv("DWF_BLOCK_ORDER");
+        const double block_mb = (double)B[0] * B[1] * B[2] * B[3] * ((double)h->Ls * 24 * 2 + 72) * real_bytes(h) / 1e6;   // in + out + links
+        double budget_mb = 80.0;                                // of the 126 MB L2 (DWF_L2_BUDGET_MB overrides: tuning)
+        if (const char* e = getenv("DWF_L2_BUDGET_MB")) budget_mb = std::max(1.0, atof(e));
         if (ord && !strcmp(ord, "morton")) {
             auto code = [](const std::array<int, 4>& b) {
                 unsigned long long c = 0;
@@ -126,6 +136,23 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
                 return c;
             };
             std::stable_sort(blocks.begin(), blocks.end(), [&](const std::array<int, 4>& x, const std::array<int, 4>& y) { return code(x) < code(y); });
+        } else if (ord && !strcmp(ord, "panel")) {
+            // panel extents: start from the whole cross-section and halve the largest extent (keeping divisibility) until it fits
+            int P[3] = {nb[0], nb[1], nb[2]};
+            while ((double)P[0] * P[1] * P[2] * block_mb > budget_mb) {
+                int best = -1;
+                for (int d = 0; d < 3; d++) if (P[d] > 1 && (best < 0 || P[d] > P[best])) best = d;
+                if (best < 0) break;
+                int q = P[best] - 1;                            // largest smaller divisor of nb[best]
+                while (q > 1 && nb[best] % q != 0) q--;
+                P[best] = q;
+            }
+            auto key = [&](const std::array<int, 4>& b) {
+                const long long panel = (b[0] / P[0]) + (long long)(nb[0] / P[0]) * ((b[1] / P[1]) + (long long)(nb[1] / P[1]) * (b[2] / P[2]));
+                const long long inside = (b[0] % P[0]) + (long long)P[0] * ((b[1] % P[1]) + (long long)P[1] * (b[2] % P[2]));
+                return (panel * nb[3] + b[3]) * ((long long)P[0] * P[1] * P[2]) + inside;
+            };
+            std::stable_sort(blocks.begin(), blocks.end(), [&](const std::array<int, 4>& x, const std::array<int, 4>& y) { return key(x) < key(y); });
         }
     }
     for (const auto& bb : blocks) { const int bx = bb[0], by = bb[1], bz = bb[2], bt = bb[3];
@@ -179,7 +206,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
     h->device = dev;
     h->no_fuse_moo = getenv("DWF_NO_FUSE_MOOINV") != nullptr;
     h->no_fuse_norm = getenv("DWF_NO_FUSE_NORM") != nullptr;
-    { const char* genv = getenv("DWF_CG_GRAPH"); h->cg_graph = genv ? atoi(genv) : 0; }
+    { const char* genv = getenv("DWF_CG_GRAPH"); h->cg_graph = genv ? atoi(genv) : -1; }
     std::vector<int> lex, nbr;
     build_tables(h, lex, nbr);
     h->rhs_chunk = 1;      // measured on B200 (16^3x32x16 fp32): 1 is fastest (132 us per rhs at nrhs 12; 4: 142 us): a chunk of c rhs needs c slabs of the lattice in L2
@@ -211,6 +238,7 @@ extern "C" int dwf_destroy(dwf_handle h) {
     if (!h) return DWF_EINVAL;
     cudaFree(h->gauge); cudaFree(h->glinks); cudaFree(h->inv_lex); cudaFree(h->nbr); cudaFree(h->lex); cudaFree(h->partial); cudaFree(h->scal); cudaFree(h->ticket);
     if (h->scal_host) cudaFreeHost(h->scal_host);
+    if (h->cg_exec) cudaGraphExecDestroy(h->cg_exec);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     delete h;
     return DWF_OK;
@@ -866,27 +894,38 @@ static int cg_schur_impl(dwf_handle h, const void* b_even, void* x_even, int ite
     if (b_even == x_even) FAIL(h, DWF_EINVAL, "b == x");
     if (!h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
     if (int rc = need_ws(h, (kind ? 8 : 5) * half_bytes(h, nrhs))) return rc;
-    // The host loop only enqueues (alpha, beta live on the device).  DWF_CG_GRAPH=1 captures the whole solve into a
-    // CUDA graph and launches it as one unit; measured on B200 (8^4x16: 7037 vs 7388 it/s, 16^3x32x16: no change)
-    // the plain stream launches are already back to back, so the graph is off by default.
-    const bool use_graph = h->cg_graph != 0 && iters > 0;
+    // The host loop only enqueues (alpha, beta live on the device).  At launch-bound sizes (a half field of a few MB: configs[1],
+    // where an iteration is five kernels of a few microseconds) the whole solve is captured once into a CUDA graph, kept
+    // instantiated in the handle, and re-launched as one unit whenever the same (b, x, iters, nrhs, workspace) recur; other
+    // arguments re-capture.  DWF_CG_GRAPH=0 / 1 forces it off / on for every size.
+    const bool small = half_bytes(h, nrhs) * (kind ? 2 : 1) <= ((size_t)8 << 20);
+    const bool use_graph = iters > 0 && (h->cg_graph == 1 || (h->cg_graph < 0 && small));
     int rc;
     if (use_graph) {
         cudaStream_t user = h->stream;
-        cudaGraph_t graph = nullptr; cudaGraphExec_t exec = nullptr;
-        CUDA_TRY(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
-        h->stream = h->cap_stream;
-        rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind) : cg_t<double>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind);
-        h->stream = user;
-        cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
-        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
-        if (e != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
-        e = cudaGraphInstantiate(&exec, graph, 0);
-        if (e == cudaSuccess) e = cudaGraphLaunch(exec, user);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(user);
-        if (exec) cudaGraphExecDestroy(exec);
-        cudaGraphDestroy(graph);
-        if (e != cudaSuccess) FAIL(h, DWF_ECUDA, "CUDA graph of the CG loop: %s", cudaGetErrorString(e));
+        const bool hit = h->cg_exec && h->cg_b == b_even && h->cg_x == x_even && h->cg_ws == h->ws && h->cg_ws_bytes == h->ws_bytes
+                      && h->cg_iters == iters && h->cg_nrhs == nrhs && h->cg_kind == kind;
+        if (!hit) {
+            if (h->cg_exec) { cudaGraphExecDestroy(h->cg_exec); h->cg_exec = nullptr; }
+            cudaGraph_t graph = nullptr;
+            CUDA_TRY(h, cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+            h->stream = h->cap_stream;
+            const long long launches0 = h->launches;
+            rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind) : cg_t<double>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind);
+            h->stream = user;
+            cudaError_t e = cudaStreamEndCapture(h->cap_stream, &graph);
+            if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+            e = cudaGraphInstantiate(&h->cg_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { h->cg_exec = nullptr; FAIL(h, DWF_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e)); }
+            h->cg_b = b_even; h->cg_x = x_even; h->cg_ws = h->ws; h->cg_ws_bytes = h->ws_bytes;
+            h->cg_iters = iters; h->cg_nrhs = nrhs; h->cg_kind = kind;
+            h->cg_launches = h->launches - launches0;
+            h->launches = launches0;                           // capture only records: the launches are counted when the graph runs
+        }
+        CUDA_TRY(h, cudaGraphLaunch(h->cg_exec, user));
+        h->launches += h->cg_launches;
     } else {
         rc = h->prec == DWF_F32 ? cg_t<float>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind) : cg_t<double>(h, b_even, x_even, iters, nrhs, 0.0, 10, nullptr, kind);
         if (rc) return rc;

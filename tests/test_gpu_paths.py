@@ -56,16 +56,33 @@ def test_fused_mooinv_vs_separate(monkeypatch, prec):
 
 
 def test_cg_graph_vs_stream(monkeypatch):
+    """The CG solve enqueued kernel by kernel (DWF_CG_GRAPH=0) and as one CUDA graph kept instantiated in the handle (the default at
+    this launch-bound size; DWF_CG_GRAPH=1 forces it): bit identical, on a cache miss, on a hit, and after the arguments changed."""
     L, Ls, mass = (8, 8, 8, 8), 16, 0.01
+    monkeypatch.setenv("DWF_CG_GRAPH", "0")                           # read at dwf_create
     rig = Rig(L, Ls, "f32", mass, seed_U=1001, ws_nrhs=1)
     b = rig.native(gen.keep_parity(rig.spinor(1, 2001), L, 0), 0)
     x1 = rig.d.field(1, half=True, zero=True)
+    l0 = rig.d.launch_count()
     h1 = rig.d.cg_schur(b, x1, 20)
-    monkeypatch.setenv("DWF_CG_GRAPH", "1")                           # read at dwf_create
-    rig2 = Rig(L, Ls, "f32", mass, seed_U=1001, ws_nrhs=1)
-    x2 = rig2.d.field(1, half=True, zero=True)
-    h2 = rig2.d.cg_schur(b, x2, 20)
-    assert h1 == h2 and bool((x1 == x2).all())        # deterministic reductions: bit identical
+    n_stream = rig.d.launch_count() - l0
+    for env in ("1", None):
+        if env is None:
+            monkeypatch.delenv("DWF_CG_GRAPH")
+        else:
+            monkeypatch.setenv("DWF_CG_GRAPH", env)
+        rig2 = Rig(L, Ls, "f32", mass, seed_U=1001, ws_nrhs=1)
+        x2 = rig2.d.field(1, half=True, zero=True)
+        l0 = rig2.d.launch_count()
+        h2 = rig2.d.cg_schur(b, x2, 20)                               # miss: capture + instantiate + launch
+        assert rig2.d.launch_count() - l0 == n_stream                 # the graph's kernels are counted once, when it runs
+        assert h1 == h2 and bool((x1 == x2).all())                    # deterministic reductions: bit identical
+        x2.zero_()
+        assert rig2.d.cg_schur(b, x2, 20) == h1 and bool((x1 == x2).all())     # hit: the kept graph is re-launched
+        x3 = rig2.d.field(1, half=True, zero=True)
+        assert rig2.d.cg_schur(b, x3, 20) == h1 and bool((x1 == x3).all())     # other x: re-captured
+        h10 = rig2.d.cg_schur(b, x3.zero_(), 10)                      # other iteration count: re-captured
+        assert h10 == h1[:11]
 
 
 @pytest.mark.parametrize("prec", ["f32", "f64"])
