@@ -435,6 +435,25 @@ def run_extras(dev, peak):
     del xs4, ys4
     d.close(); del d
     gc.collect(); torch.cuda.empty_cache()
+    # ---- Table V rows 1-2 on the synthetic 16^3x32x16 field (fp32): unpreconditioned CGNR on M^dag M and BiCGSTAB on M_PV^dag M,
+    # 20 iterations each, iterations/s and the number of full-lattice operator applies per iteration (2 and 4)
+    d = Dwf(L, LS, M5, MASS, DWF_F32, device=dev)
+    d.set_gauge(torch.from_numpy(gen.gauge_random(L, 1002)).to(torch.complex64).to(dev))
+    d.set_workspace(1)
+    g = torch.Generator(device=dev); g.manual_seed(2012)
+    bfull = d.field(1).normal_(generator=g); xfull = d.field(1, zero=True)
+    for name, fn, applies in (("cgnr_MdagM", lambda: d.cg_normal(bfull, xfull.zero_(), 20, 1), 2),
+                              ("bicgstab_MpvdagM", lambda: d.bicgstab_pv(bfull, xfull.zero_(), 20), 4)):
+        fn(); torch.cuda.synchronize(); t0 = time.perf_counter()
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        ms = (time.perf_counter() - t0) * 1e3 / 3
+        out[f"{name}_16^3x32x16_fp32"] = {"iters": 20, "ms": round(ms, 3), "iterations/s": round(21 / ms * 1e3, 1),
+                                          "full_applies_per_iteration": applies,
+                                          "GFlop/s": round(FLOP_PER_SITE * V5 * applies * 21 / ms / 1e6, 1)}
+    d.close(); del d, bfull, xfull
+    gc.collect(); torch.cuda.empty_cache()
     # ---- configs[1]: 8^4 x 16, 50 rb-CG iterations (launch-bound size), fp32 and fp64
     L8 = (8, 8, 8, 8)
     for prec, code, cdt in (("fp32", DWF_F32, torch.complex64), ("fp64", DWF_F64, torch.complex128)):
