@@ -222,18 +222,39 @@ __device__ __forceinline__ void acc_inner(double& sre, double& sim, CV<double> x
     sim += x.re * y.im - x.im * y.re;
 }
 
-// Fixed-order combine of the 256 per-thread sums of a block into per-rhs block partials:
-// partial[(blockIdx.x * nrhs + r) * 2 + {0,1}].
-__device__ __forceinline__ void block_combine(double sre, double sim, int r, int nrhs, double* partial) {
+// Fixed-order combine of the 256 per-thread sums of a block into per-rhs block partials
+// partial[(blockIdx.x * nrhs + r) * 2 + {0,1}]  (north_star item (4): warp shuffle + block reduction).
+// When the groups of one rhs come in runs that are a multiple of 32 (BS % 32 == 0: every production layout) all lanes of a warp
+// hold the same rhs: a butterfly of shuffles reduces the warp, and thread r adds the (at most 8) warp sums of its rhs in warp
+// order.  Otherwise (narrow blocks of the generic layout) thread r walks the 256 entries of its rhs in thread order.
+__device__ __forceinline__ void block_combine(double sre, double sim, int r, int nrhs, int BS, double* partial) {
     __shared__ double s_re[256], s_im[256];
     __shared__ int s_r[256];
-    s_re[threadIdx.x] = sre; s_im[threadIdx.x] = sim; s_r[threadIdx.x] = r;
+    const int t = threadIdx.x;
+    if ((BS & 31) == 0) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            sre += __shfl_xor_sync(0xffffffffu, sre, off);
+            sim += __shfl_xor_sync(0xffffffffu, sim, off);
+        }
+        if ((t & 31) == 0) { s_re[t >> 5] = sre; s_im[t >> 5] = sim; s_r[t >> 5] = r; }
+        __syncthreads();
+        if (t < nrhs) {
+            double a = 0, b = 0;
+            const int nw = (int)blockDim.x >> 5;
+            for (int w = 0; w < nw; w++) if (s_r[w] == t) { a += s_re[w]; b += s_im[w]; }
+            partial[((size_t)blockIdx.x * nrhs + t) * 2] = a;
+            partial[((size_t)blockIdx.x * nrhs + t) * 2 + 1] = b;
+        }
+        return;
+    }
+    s_re[t] = sre; s_im[t] = sim; s_r[t] = r;
     __syncthreads();
-    if ((int)threadIdx.x < nrhs) {
+    if (t < nrhs) {
         double a = 0, b = 0;
-        for (int t = 0; t < (int)blockDim.x; t++) if (s_r[t] == (int)threadIdx.x) { a += s_re[t]; b += s_im[t]; }
-        partial[((size_t)blockIdx.x * nrhs + threadIdx.x) * 2] = a;
-        partial[((size_t)blockIdx.x * nrhs + threadIdx.x) * 2 + 1] = b;
+        for (int q = 0; q < (int)blockDim.x; q++) if (s_r[q] == t) { a += s_re[q]; b += s_im[q]; }
+        partial[((size_t)blockIdx.x * nrhs + t) * 2] = a;
+        partial[((size_t)blockIdx.x * nrhs + t) * 2 + 1] = b;
     }
 }
 
@@ -251,7 +272,7 @@ inner_kernel(const typename Prec<R>::G* __restrict__ x, const typename Prec<R>::
         if constexpr (NORM) acc_inner(sre, sim, xx, xx);
         else                acc_inner(sre, sim, xx, unpack(ldg_nc(y + e)));
     }
-    block_combine(sre, sim, r, nrhs, partial);
+    block_combine(sre, sim, r, nrhs, BS, partial);
 }
 
 // out[r*ostride + {0,1}] = sum over blocks of partial.  One block of 256 threads per rhs: thread t adds the partials
@@ -293,7 +314,7 @@ cg_init_kernel(const typename Prec<R>::G* __restrict__ b, const typename Prec<R>
         r[e] = pack(rr); p[e] = pack(rr);
         acc_inner(sre, sim, rr, rr);
     }
-    block_combine(sre, sim, rhs, nrhs, partial);
+    block_combine(sre, sim, rhs, nrhs, BS, partial);
 }
 
 template <typename R>
@@ -315,7 +336,7 @@ cg_update_xr_kernel(typename Prec<R>::G* x, typename Prec<R>::G* r, const typena
         x[e] = pack(xx); r[e] = pack(rv);
         acc_inner(sre, sim, rv, rv);
     }
-    block_combine(sre, sim, rhs, nrhs, partial);
+    block_combine(sre, sim, rhs, nrhs, BS, partial);
 }
 
 // fused iteration (dwf_api.cu cg_t): x += alpha p ; p = r + beta p   (r already updated by the adjoint Schur launch)
