@@ -144,7 +144,8 @@ int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs, int half)
 
 /* `iters` iterations of Hestenes-Stiefel CG on M_pc^dag M_pc x = b (eq. 9), nrhs = 1, even half
  * fields.  x_even holds x_0 on entry and x_iters on return.  resid2_hist_host (may be NULL) receives
- * iters+1 values |r_k|^2.  Uses the workspace (5 half fields).  Synchronises at the end only. */
+ * iters+1 values |r_k|^2.  Uses the workspace (5 half fields).  Synchronises at the end only.  At launch-bound sizes (a half field
+ * of at most 8 MB) the solve is captured into a CUDA graph that the handle keeps and re-launches while (b, x, iters, workspace) recur. */
 int dwf_cg_schur(dwf_handle h, const void* b_even, void* x_even, int iters, double* resid2_hist_host);
 
 /* The same CG on nrhs right-hand sides in lock step (one independent CG per rhs: per-rhs alpha, beta; every kernel serves all
