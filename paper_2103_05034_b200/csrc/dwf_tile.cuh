@@ -280,16 +280,25 @@ hop_tile_kernel(const HopArgs<R> a) {
                     R pw = R(1);
 #pragma unroll
                     for (int j = 0; j < LS; j++) { b[j] = fma(pw, v0, b[j]); pw *= kappa; }
-                    H* orow = reinterpret_cast<H*>(obase_t + (size_t)row * K);
+                    // back into the same row of the transposition buffer (only this task touches its half of the row) ...
+                    H* s_w = reinterpret_cast<H*>(s_t);
 #pragma unroll
                     for (int kk = 0; kk < K; kk++) {
                         H g;
                         if constexpr (VL == 2) { g.x = down ? b[2 * kk] : b[2 * kk + 1]; g.y = down ? b[2 * kk + 1] : b[2 * kk]; }
                         else g = b[kk];
-                        orow[(down ? kk : K - 1 - kk) * 2 + part] = g;
+                        s_w[(row * (K + 1) + (down ? kk : K - 1 - kk)) * 2 + part] = g;
                     }
                 }
-                release_buffers();                             // the solver's reads of the buffer are complete (values consumed)
+                __syncthreads();
+                // ... and out in the lane layout: the same whole-line streaming stores as every other epilogue (storing the rows
+                // straight from the tasks costs 16 half-used sectors per warp instruction: Schur K1 91 us instead of 7x us)
+                {
+                    G* o = obase_t + (size_t)ls * BS + k;
+#pragma unroll
+                    for (int c = 0; c < 12; c++) __stcs(o + c * K, s_t[(ls * 12 + c) * (K + 1) + k]);
+                }
+                release_buffers();                             // the reads of the buffer are complete (values consumed)
                 continue;
             }
         }
