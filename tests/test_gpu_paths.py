@@ -4,6 +4,7 @@ oracle in test_gpu_parity.py / test_gpu_fullsize.py through whichever path is th
   * tiled persistent stencil (dwf_tile.cuh)  vs  generic stencil (dwf_hop.cuh)      DWF_NO_TILE=1
   * Schur K1 with the fused M_oo^-1 epilogue vs  separate mooinv_kernel            DWF_NO_FUSE_MOOINV=1
   * CG enqueued on the stream                vs  CG captured into a CUDA graph     DWF_CG_GRAPH=1
+  * 16- / 32- / 64-site tiles of the tiled stencil (small lattices default to 16)   DWF_TILE=bx,by,bz,bt
 """
 import numpy as np
 import pytest
@@ -85,14 +86,47 @@ def test_cg_graph_vs_stream(monkeypatch):
         assert h10 == h1[:11]
 
 
-@pytest.mark.parametrize("prec", ["f32", "f64"])
-def test_repeatable_bit_for_bit(prec):
+def test_tile_sizes_agree(oracle, monkeypatch):
+    """fp32, Ls 16: lattices with fewer than two 32-site tiles per SM default to 16-site tiles (dwf_api.cu build_tables); the
+    32-site geometry (the production one at 16^3x32) and the 64-site one are forced through DWF_TILE.  The per-site arithmetic
+    does not depend on the tile shape: operator results are bit identical; the CG residual history (reduction order differs)
+    agrees to rounding; the default is anchored to the oracle."""
+    L, Ls, mass, nrhs = (8, 8, 8, 8), 16, 0.01, 2
+    outs, hists = {}, {}
+    psi = None
+    for tag, env in (("default", None), ("ts32", "4,4,2,2"), ("ts64", "4,4,4,2"), ("ts16", "4,2,2,2")):
+        if env:
+            monkeypatch.setenv("DWF_TILE", env)
+        rig = Rig(L, Ls, "f32", mass, seed_U=51, ws_nrhs=nrhs)
+        if psi is None:
+            psi = rig.spinor(nrhs, 52)
+        pe = gen.keep_parity(psi, L, 0)
+        outs[tag] = [rig.apply(DWF_DDW, psi), rig.apply(DWF_HDW, psi), rig.apply(DWF_DDW | DWF_DAGGER, psi),
+                     rig.apply(DWF_SCHUR_EO, pe, half=True), rig.apply(DWF_SCHUR_EO | DWF_DAGGER, pe, half=True)]
+        cheb = rig.d.field(nrhs)
+        rig.d.chebyshev(4, 0.01, 70.0, rig.native(psi), cheb, nrhs)
+        outs[tag].append(rig.canonical(cheb, nrhs))
+        b = rig.native(gen.keep_parity(psi[:1], L, 0), 0)
+        hists[tag] = np.array(rig.d.cg_schur(b, rig.d.field(1, half=True, zero=True), 12))
+    assert np.array_equal(outs["default"][0], outs["ts16"][0])          # the default IS the 16-site geometry at this size
+    for tag in ("ts32", "ts64", "ts16"):
+        for a, b in zip(outs["default"], outs[tag]):
+            assert np.array_equal(a, b), tag
+        assert np.max(np.abs(hists[tag] - hists["default"]) / hists["default"]) < 1e-5, tag
+    assert rel_l2(outs["default"][0], oracle.ddw(rig.U, psi, M5, mass)) < 1e-5
+    assert rel_l2(outs["default"][3], oracle.mpc(rig.U, gen.keep_parity(psi, L, 0), M5, mass)) < 1e-5
+
+
+@pytest.mark.parametrize("prec,tile", [("f32", None), ("f32", "4,4,2,2"), ("f64", None)])
+def test_repeatable_bit_for_bit(monkeypatch, prec, tile):
     """The persistent kernel hands its shared-memory buffers over through mbarriers and an atomic counter: a race there would
     show up as run-to-run differences.  30 applies of H_DW (+ the Chebyshev pair, + the fused Schur) on one input at a size with
     many work items per CTA must be bit identical."""
     import torch
     from paper_2103_05034_b200 import DWF_SCHUR_EO
     L, Ls, nrhs = (16, 16, 8, 8), 16, 2
+    if tile:
+        monkeypatch.setenv("DWF_TILE", tile)              # the 32-site geometry of the bench lattice (this lattice defaults to 16)
     rig = Rig(L, Ls, prec, 0.01, seed_U=81, ws_nrhs=nrhs)
     g = torch.Generator(device="cuda"); g.manual_seed(82)
     x = rig.d.field(nrhs).normal_(generator=g)
