@@ -42,6 +42,7 @@ struct dwf_ctx {
     double* scal;         // device scalars (reduction results, CG history)
     double* scal_host;    // pinned mirror
     int sm_count, device;
+    size_t l2_bytes;      // cudaDevAttrL2CacheSize (picks the t-extent of the lattice blocks, build_tables)
     bool no_fuse_moo, no_fuse_norm;   // DWF_NO_FUSE_MOOINV / DWF_NO_FUSE_NORM, read once at dwf_create (the unfused reference path)
     int cg_graph;         // DWF_CG_GRAPH, read once at dwf_create: 0 never, 1 always, unset (-1): launch-bound sizes only
     // the instantiated CUDA graph of the last CG solve and the arguments it was captured for (re-launched when they recur)
@@ -98,6 +99,15 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     // small lattices: fewer 32-site tiles than two per SM leave most of the GPU idle in every launch -- 16-site tiles double the
     // work items (measured on B200, 8^4 x 16 fp32 red-black CG: 23.6k -> 28.5k iterations/s)
     if (h->V4h / 32 < 2LL * h->sm_count) T[1] = 2;
+    // Blocks are swept x fastest, t slowest, so the -t halo of a block layer is re-read one layer later.  When two layers of
+    // t-extent 2 (input + output + gathered links) fit L2 the thin layer keeps that halo resident: measured on B200 at 16^3x32x16,
+    // block 4,4,4,2 against 4,4,4,4: D_DW fp32 130.5 -> 127.0 us, fp64 304 -> 281 us, H_DW fp64 nrhs 12 3.81 -> 3.67 ms.  When a layer is
+    // far larger than L2 (48^3x96x24: 510 MB) every t face misses anyway and the taller block halves the faces: 4,4,4,4 21.4 ms,
+    // 4,4,4,2 25.1 ms, 4,4,4,8 23.7 ms (larger blocks lengthen the y/z reuse distance instead).
+    {
+        const double layer2 = (double)L[0] * L[1] * L[2] * 2 * ((double)h->Ls * 24 * 2 + 2 * 72) * real_bytes(h);
+        if (2 * layer2 <= (double)h->l2_bytes) B[3] = 2;
+    }
     auto parse = [](const char* name, int* v) {
         if (const char* env = getenv(name)) { int b[4]; if (sscanf(env, "%d,%d,%d,%d", &b[0], &b[1], &b[2], &b[3]) == 4) for (int i = 0; i < 4; i++) v[i] = b[i]; }
     };
@@ -207,6 +217,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
         delete h; return DWF_ECUDA;
     }
     h->device = dev;
+    { int l2 = 0; if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) != cudaSuccess || l2 <= 0) l2 = 64 << 20; h->l2_bytes = (size_t)l2; }
     h->no_fuse_moo = getenv("DWF_NO_FUSE_MOOINV") != nullptr;
     h->no_fuse_norm = getenv("DWF_NO_FUSE_NORM") != nullptr;
     { const char* genv = getenv("DWF_CG_GRAPH"); h->cg_graph = genv ? atoi(genv) : -1; }
