@@ -99,7 +99,10 @@ int dwf_export(dwf_handle h, const void* native_dev, void* canonical_dev, int nr
 int dwf_apply(dwf_handle h, int op, const void* in, void* out, int nrhs);
 
 /* Same operator (every op of dwf_apply, DWF_DAGGER included), end to end from HOST canonical arrays: H2D copy, import,
- * apply, export, D2H copy (synchronises).  Workspace: 4 half fields of staging + the operator's own need.  For the
+ * apply, export, D2H copy (synchronises).  Workspace: 4 half fields of staging + the operator's own need.  With 6 half fields the
+ * one-launch full-lattice operators (DHOP, DDW, DPV, HDW) run pipelined over chunks of t-slices (host -> device copy of chunk c+1,
+ * kernels of chunk c and device -> host copy of chunk c-1 at the same time; in_host != out_host; lattices with at least three
+ * t-layers of blocks), which roughly halves the time of a PCIe-bound call; DWF_NO_HOST_PIPELINE=1 keeps the serial path.  For the
  * half-field ops SCHUR_EO/SCHUR_EO_ALT/MEE/MOOINV the arrays are full-lattice canonical arrays of which only the even
  * sites are read; the odd sites of out_host are written as zero. */
 int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* out_host, int nrhs);

@@ -49,6 +49,9 @@ struct dwf_ctx {
     long long cg_launches;
     cudaGraphExec_t cg_exec; const void* cg_b; void* cg_x; void* cg_ws; size_t cg_ws_bytes; int cg_iters, cg_nrhs, cg_kind;
     long long blk_sites;  // sites per parity in one lattice block of the native site order
+    int blk_t;            // t-extent of a lattice block; 0 when the block order is not lexicographic with t slowest (no t-layers)
+    cudaStream_t io_in, io_out;          // dwf_apply_host pipeline: H2D and D2H streams, created on first use
+    cudaEvent_t io_ev[2 * 16 + 1];       //   chunk c arrived / chunk c exported / the handle's stream reached the call
     int tile_sites;       // sites per parity in one tile of the native site order (0: lattice is not made of whole tiles)
     int sg_shift;         // block order [site group][rhs][site in group]: log2(group size)
     int rhs_chunk;        // right-hand sides per stencil launch
@@ -118,6 +121,7 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     if ((T[0] * T[1] * T[2] * T[3]) % 2 != 0) for (int i = 0; i < 4; i++) T[i] = B[i];
     const long long V4 = h->V4, V4h = h->V4h;
     h->blk_sites = (long long)B[0] * B[1] * B[2] * B[3] / 2;
+    h->blk_t = (getenv("DWF_BLOCK_ORDER") == nullptr && L[3] % B[3] == 0) ? B[3] : 0;   // lexicographic block order: t-layers of blocks are contiguous site ranges
     const int tsites = T[0] * T[1] * T[2] * T[3] / 2;
     bool whole = true;
     for (int i = 0; i < 4; i++) whole = whole && (L[i] % T[i] == 0);
@@ -254,6 +258,7 @@ extern "C" int dwf_destroy(dwf_handle h) {
     if (h->scal_host) cudaFreeHost(h->scal_host);
     if (h->cg_exec) cudaGraphExecDestroy(h->cg_exec);
     if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+    if (h->io_in) { cudaStreamDestroy(h->io_in); cudaStreamDestroy(h->io_out); for (cudaEvent_t e : h->io_ev) if (e) cudaEventDestroy(e); }
     delete h;
     return DWF_OK;
 }
@@ -308,17 +313,21 @@ extern "C" int dwf_set_gauge(dwf_handle h, const void* U) {
     return DWF_OK;
 }
 
+// site0 .. site1: the sites (native order, per parity) this launch converts; site1 = 0: all
 template <typename R, bool IMPORT>
-static int reorder_spinor(dwf_ctx* h, const void* canon_in, void* canon_out, void* native, int nrhs, int parity) {
+static int reorder_spinor(dwf_ctx* h, const void* canon_in, void* canon_out, void* native, int nrhs, int parity,
+                          long long site0 = 0, long long site1 = 0) {
     using G = typename Prec<R>::G;
     const long long per_parity = half_groups(h, nrhs);
     G* n0; G* n1; const int* l0; const int* l1; unsigned ny;
     if (parity < 0) { n0 = (G*)native; n1 = (G*)native + per_parity; l0 = h->lex; l1 = h->lex + h->V4h; ny = 2; }
     else            { n0 = n1 = (G*)native; l0 = l1 = h->lex + (size_t)parity * h->V4h; ny = 1; }
-    const long long pairs = h->V4h * nrhs;                                       // one warp per (site, rhs) block
+    if (site1 == 0) site1 = h->V4h;
+    const long long pairs = (site1 - site0) * nrhs;                              // one warp per (site, rhs) block
     dim3 grid((unsigned)((pairs + 3) / 4), ny);
     const size_t dsm = 4 * 24 * (size_t)h->Ls * sizeof(R);
-    reorder_spinor_kernel<R, IMPORT><<<grid, 128, dsm, h->stream>>>((const R*)canon_in, (R*)canon_out, n0, n1, l0, l1, h->V4h, h->V4, h->Ls, nrhs, h->sg_shift);
+    reorder_spinor_kernel<R, IMPORT><<<grid, 128, dsm, h->stream>>>((const R*)canon_in, (R*)canon_out, n0, n1, l0, l1, h->V4h, h->V4, h->Ls, nrhs, h->sg_shift,
+                                                                    site0 * nrhs, site1 * nrhs);
     LAUNCH_CHECK(h);
     return DWF_OK;
 }
@@ -355,6 +364,7 @@ struct HopCall {            // precision-independent description of one launch
     double* norm_out;       // tiled HM_HOP_SELF (not dag) and HM_HOP_SELF_AXPBY_NORM, nrhs = 1: also *norm_out = |out|^2 (device), summed
                             // inside the launch (dwf_tile.cuh NORM epilogue)
     const double* ax_num; const double* ax_den;   // HM_HOP_SELF_AXPBY_NORM: ax_a = -(*ax_num / *ax_den), read on the device
+    long long site0, site1;  // output sites (native order, per parity) of this launch, whole lattice blocks; site1 = 0: all
 };
 
 // Is the tiled persistent stencil (dwf_tile.cuh) instantiated for this handle?  Lattice made of whole tiles, Ls 16 (16- or
@@ -364,6 +374,13 @@ static bool tiled_ok(const dwf_ctx* h) {
     if (h->tile_sites == 64 && !(h->Ls == 16 && h->prec == DWF_F32)) return false;
     if (!(h->Ls == 16 || (h->Ls == 24 && (h->tile_sites == 16 || h->prec == DWF_F32)))) return false;
     return 2 * (h->V4h / h->tile_sites + h->blk_sites) * (long long)h->rhs_chunk < (1LL << 31);
+}
+
+// Partial launches (HopCall::site0/site1) cover whole parity-interleave chunks: this many sites per parity
+static long long partial_unit(const dwf_ctx* h) {
+    const int K = h->Ls / vl(h);
+    const long long GS = tiled_ok(h) ? h->tile_sites : std::min(HOP_THREADS / 8, HOP_THREADS / K);
+    return std::max<long long>(1, h->blk_sites / GS) * GS;
 }
 
 template <typename R>
@@ -390,6 +407,12 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.chunk_groups = std::max<long long>(1, h->blk_sites / a.GS);             // parity interleave unit = one lattice block
     long long groups = a.ngroups;
     if (k.nslots == 2) groups = 2 * ((a.ngroups + a.chunk_groups - 1) / a.chunk_groups) * a.chunk_groups;
+    long long group0 = 0;                                                       // first site group (CTA of the generic kernel / tile) of a partial launch
+    if (k.site1) {
+        const long long unit = a.chunk_groups * a.GS;                           // sites per parity-interleave chunk
+        if (k.site0 % unit || k.site1 % unit || k.site1 > h->V4h) FAIL(h, DWF_EINVAL, "partial launch: site range must be whole lattice blocks");
+        group0 = k.site0 / a.GS * k.nslots; groups = k.site1 / a.GS * k.nslots;
+    }
     cudaStream_t st = h->stream;
     const size_t lsite = 144 * sizeof(R) + 16;
     a.glinks[0] = (const R*)h->glinks;
@@ -412,7 +435,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
             if (e_ != cudaSuccess) FAIL(h, DWF_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(e_)); \
             attr_done |= 1ull << (h->device & 63); \
         } \
-        const long long ctas = std::min<long long>(a.nitems, (long long)h->sm_count * TG::MIN_CTAS); \
+        const long long ctas = std::min<long long>(a.nitems - a.item0, (long long)h->sm_count * TG::MIN_CTAS); \
         kern<<<(unsigned)ctas, TG::THREADS, TG::SMEM_BYTES, st>>>(a); } while (0)
 #define HOPM(LS) \
     switch (k.mode) { \
@@ -441,8 +464,8 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     const int RC = h->rhs_chunk;
     for (int r0 = 0; r0 < k.nrhs; r0 += RC) {
         a.r0 = r0; a.rn = std::min(RC, k.nrhs - r0);
-        a.nitems = groups * a.rn;
-        dim3 grid((unsigned)(groups * a.rn));
+        a.item0 = group0 * a.rn; a.nitems = groups * a.rn;
+        dim3 grid((unsigned)((groups - group0) * a.rn));
         // compile-time Ls for the production sizes (tiled when the lattice allows), runtime Ls otherwise
         if (h->Ls == 16)      { if (TS == 64) { if constexpr (sizeof(R) == 4) { TILEM(16, 64) } } else if (TS == 32) { TILEM(16, 32) } else if (TS == 16) { TILEM(16, 16) } else { HOPM(16) } }
         else if (h->Ls == 24) { if (TS == 16) { TILEM(24, 16) } else if (TS == 32) { if constexpr (sizeof(R) == 4) { TILEM(24, 32) } } else { HOPM(24) } }
@@ -483,7 +506,8 @@ static int launch_mooinv(dwf_ctx* h, const void* in, void* out, int nrhs, double
 
 // full-lattice operator:  out_p = c_hop hop(in_{1-p}) [+ self(in_p)] for both parities, one launch
 static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, const void* in, void* out, int nrhs,
-                   double ax_a = 0, const void* y = nullptr, double ax_b = 0, const void* z = nullptr, double ax_c = 0) {
+                   double ax_a = 0, const void* y = nullptr, double ax_b = 0, const void* z = nullptr, double ax_c = 0,
+                   long long site0 = 0, long long site1 = 0) {
     const size_t hb = half_bytes(h, nrhs);
     HopCall k{};
     k.mode = mode; k.dag = dag; k.nslots = 2; k.parity0 = 0; k.nrhs = nrhs;
@@ -495,6 +519,7 @@ static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, co
         k.z[p] = z ? (const char*)z + (size_t)p * hb : nullptr;
     }
     k.c_hop = c_hop; k.mass = mass; k.ax_a = ax_a; k.ax_b = ax_b; k.ax_c = ax_c;
+    k.site0 = site0; k.site1 = site1;
     return launch_hop(h, k);
 }
 
@@ -1176,6 +1201,57 @@ extern "C" int dwf_solve_mixed(dwf_handle h64, dwf_handle h32, const void* eta, 
 // Workspace use: [0, F) canonical staging / native out, [F, 2F) native in / canonical out, [2F, ...) the operator's own scratch
 // (SCHUR_EO: 1 half field, SCHUR_EO_ALT and MPVDAG_M: 2)
 // ------------------------------------------------------------------------------------------------
+// dwf_apply_host for the one-launch full-lattice operators, pipelined over chunks of t-slices: while chunk c is converted and
+// applied, chunk c+1 arrives over PCIe and chunk c-1 leaves (the two copy directions run at the same time).  The canonical
+// layout [rhs][s][t][...] makes a t-range one 2-D copy (rows = (rhs, s)); in the native order (lexicographic blocks, t slowest) it
+// is a contiguous range of sites and of work items.  A chunk's operator needs its two t-neighbour chunks imported.
+// Buffers: A = canonical in, then canonical out chunk by chunk; B = native in; C = native out (6 half fields).
+static int apply_host_pipelined(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, const void* in_host, void* out_host, int nrhs, int nc) {
+    const size_t hb = half_bytes(h, nrhs), fb = 2 * hb, R = real_bytes(h);
+    char* A = (char*)h->ws; char* B = A + fb; char* C = B + fb;
+    if (!h->io_in) {
+        CUDA_TRY(h, cudaStreamCreateWithFlags(&h->io_in, cudaStreamNonBlocking));
+        CUDA_TRY(h, cudaStreamCreateWithFlags(&h->io_out, cudaStreamNonBlocking));
+        for (cudaEvent_t& e : h->io_ev) CUDA_TRY(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    cudaEvent_t* ev_in = h->io_ev; cudaEvent_t* ev_out = h->io_ev + 16; cudaEvent_t ev_start = h->io_ev[32];
+    const int Lt = h->L[3], tc = Lt / nc;                                        // t-slices per chunk
+    const size_t slice = (size_t)h->V4 / Lt * 24 * R;                           // one t-slice of one (rhs, s) row
+    const size_t pitch = slice * Lt, width = slice * tc;
+    const size_t rows = (size_t)nrhs * h->Ls;
+    const long long sc = h->V4h / nc;                                            // sites per parity per chunk
+    cudaStream_t st = h->stream;
+    CUDA_TRY(h, cudaEventRecord(ev_start, st));                                  // earlier work on the handle's stream may still use the workspace
+    CUDA_TRY(h, cudaStreamWaitEvent(h->io_in, ev_start, 0));
+    CUDA_TRY(h, cudaStreamWaitEvent(h->io_out, ev_start, 0));
+    for (int c = 0; c < nc; c++) {
+        CUDA_TRY(h, cudaMemcpy2DAsync(A + c * width, pitch, (const char*)in_host + c * width, pitch, width, rows, cudaMemcpyHostToDevice, h->io_in));
+        CUDA_TRY(h, cudaEventRecord(ev_in[c], h->io_in));
+    }
+    auto run_chunk = [&](int c) -> int {                                         // operator, export and D2H of chunk c
+        if (int rc = full_op(h, mode, dag, c_hop, mass, B, C, nrhs, 0, nullptr, 0, nullptr, 0, c * sc, (c + 1) * sc)) return rc;
+        const int rc = h->prec == DWF_F32 ? reorder_spinor<float, false>(h, nullptr, A, C, nrhs, -1, c * sc, (c + 1) * sc)
+                                          : reorder_spinor<double, false>(h, nullptr, A, C, nrhs, -1, c * sc, (c + 1) * sc);
+        if (rc) return rc;
+        CUDA_TRY(h, cudaEventRecord(ev_out[c], st));
+        CUDA_TRY(h, cudaStreamWaitEvent(h->io_out, ev_out[c], 0));
+        CUDA_TRY(h, cudaMemcpy2DAsync((char*)out_host + c * width, pitch, A + c * width, pitch, width, rows, cudaMemcpyDeviceToHost, h->io_out));
+        return DWF_OK;
+    };
+    for (int c = 0; c < nc; c++) {
+        CUDA_TRY(h, cudaStreamWaitEvent(st, ev_in[c], 0));
+        const int rc = h->prec == DWF_F32 ? reorder_spinor<float, true>(h, A, nullptr, B, nrhs, -1, c * sc, (c + 1) * sc)
+                                          : reorder_spinor<double, true>(h, A, nullptr, B, nrhs, -1, c * sc, (c + 1) * sc);
+        if (rc) return rc;
+        if (c >= 2) { if (int rc2 = run_chunk(c - 1)) return rc2; }              // chunks c-2, c-1, c are in
+    }
+    if (int rc = run_chunk(nc - 1)) return rc;                                   // periodic in t: the last and the first chunk need each other
+    if (int rc = run_chunk(0)) return rc;
+    CUDA_TRY(h, cudaStreamSynchronize(h->io_out));
+    CUDA_TRY(h, cudaStreamSynchronize(st));
+    return DWF_OK;
+}
+
 extern "C" int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* out_host, int nrhs) {
     if (!h) return DWF_EINVAL;
     if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
@@ -1184,6 +1260,23 @@ extern "C" int dwf_apply_host(dwf_handle h, int op, const void* in_host, void* o
     const bool halfop = (base == DWF_SCHUR_EO || base == DWF_MEE || base == DWF_MOOINV || base == DWF_SCHUR_EO_ALT);
     if (base != DWF_MEE && base != DWF_MOOINV && !h->have_gauge) FAIL(h, DWF_ENOGAUGE, "dwf_set_gauge has not been called");
     const size_t hb = half_bytes(h, nrhs), fb = 2 * hb;
+    // One-launch full-lattice operators with 6 half fields of workspace: copies pipelined against the kernels in chunks of t-slices
+    // (at least 3 chunks of whole block layers, at most 16).  Everything else: the serial path below.
+    if ((base == DWF_DHOP || base == DWF_DDW || base == DWF_DPV || base == DWF_HDW) && h->blk_t > 0 && h->ws
+        && h->ws_bytes >= 3 * fb && in_host != out_host && !getenv("DWF_NO_HOST_PIPELINE")) {
+        const int layers = h->L[3] / h->blk_t;
+        int nc = 0;
+        for (int n = std::min(layers, 16); n >= 3; n--) if (layers % n == 0) { nc = n; break; }
+        if (nc && (h->V4h / nc) % partial_unit(h) == 0) {
+            const bool dag = (op & DWF_DAGGER) != 0;
+            switch (base) {
+                case DWF_DHOP: return apply_host_pipelined(h, HM_HOP, dag, 1.0, h->mass, in_host, out_host, nrhs, nc);
+                case DWF_DDW:  return apply_host_pipelined(h, HM_HOP_SELF, dag, -0.5, h->mass, in_host, out_host, nrhs, nc);
+                case DWF_DPV:  return apply_host_pipelined(h, HM_HOP_SELF, dag, -0.5, 1.0, in_host, out_host, nrhs, nc);
+                default:       return apply_host_pipelined(h, HM_HOP_SELF_G5, false, -0.5, h->mass, in_host, out_host, nrhs, nc);
+            }
+        }
+    }
     // scratch of the operator itself, behind the two staging fields
     const size_t op_ws = (base == DWF_SCHUR_EO) ? hb : (base == DWF_SCHUR_EO_ALT || base == DWF_MPVDAG_M) ? 2 * hb : 0;
     if (int rc = need_ws(h, 2 * fb + op_ws)) return rc;

@@ -17,15 +17,15 @@ __global__ void __launch_bounds__(128)
 reorder_spinor_kernel(const R* __restrict__ canon_in, R* __restrict__ canon_out,
                       typename Prec<R>::G* native0, typename Prec<R>::G* native1,
                       const int* __restrict__ lex0, const int* __restrict__ lex1,
-                      long long V4h, long long V4, int Ls, int nrhs, int sg_shift) {
+                      long long V4h, long long V4, int Ls, int nrhs, int sg_shift, long long wid0, long long wid1) {
     using G = typename Prec<R>::G;
     constexpr int VL = Prec<R>::VL;
     extern __shared__ __align__(16) unsigned char smem_reorder[];
     const int K = Ls / VL, NG = 12 * K;                         // groups per block
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     R* buf = reinterpret_cast<R*>(smem_reorder) + (size_t)warp * 24 * Ls;
-    const long long wid = (long long)blockIdx.x * (blockDim.x >> 5) + warp;     // (site, rhs) pair of this parity
-    if (wid >= V4h * nrhs) return;                               // whole warps leave together
+    const long long wid = wid0 + (long long)blockIdx.x * (blockDim.x >> 5) + warp;   // (site, rhs) pair of this parity, in [wid0, wid1)
+    if (wid >= wid1) return;                                     // whole warps leave together
     const long long site = wid / nrhs;
     const int r = (int)(wid - site * nrhs);
     G* native = (blockIdx.y ? native1 : native0) + (size_t)blk_index(site, r, nrhs, sg_shift) * NG;

@@ -42,7 +42,8 @@ template <typename R> struct HopArgs {
     const R* glinks[2];    // [p] gathered links of parity-p sites: [site][mu][fwd 18 | bwd 18] x (-1/2), 16 B pad per site
     R sigma;               // res = sigma * hop' + self  with hop' built from the (-1/2)-scaled links
     R moo_kappa, moo_v0scale;   // fused M_oo^-1 epilogue: 1/(5-M5), kappa / (1 + m kappa^Ls)
-    long long nitems;      // work items (tile, rhs, parity slot) of this launch
+    long long item0;       // this launch covers work items item0 .. nitems-1 (a partial launch covers whole lattice blocks)
+    long long nitems;      // end of the work items (tile | site group, rhs, parity slot) of this launch
     double* norm_partial;  // NORM epilogue: |out|^2 partials [CTA][warp][2] (each warp's running sum over its items, in item order)
     double* norm_out;      // ... summed in (CTA, warp) order by the last CTA to finish and written here
     unsigned* ticket;      // ... CTA completion counter (zero on entry, reset to zero by the last CTA)
@@ -231,8 +232,9 @@ hop_kernel(const HopArgs<R> a) {
     __shared__ __align__(16) R s_link[HOP ? (HOP_THREADS / 8) * SITE : 4];
 
     // ---- which (output parity slot, site group, rhs) is this CTA? -------------------------------------
-    long long gg = (long long)blockIdx.x / a.rn;              // site group, maybe across both slots
-    const int r = a.r0 + (int)(blockIdx.x - gg * a.rn);
+    const long long bid = a.item0 + blockIdx.x;
+    long long gg = bid / a.rn;                                // site group, maybe across both slots
+    const int r = a.r0 + (int)(bid - gg * a.rn);
     int pi = 0;
     if (a.nslots == 2) {                                      // chunks of chunk_groups alternate between the parities
         const long long q = gg / (2 * a.chunk_groups);

@@ -157,7 +157,7 @@ hop_tile_kernel(const HopArgs<R> a) {
         bulk_g2s(smem + 128 + ib * TG::INT_STRIDE, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int + ib);
     };
 
-    long long w = blockIdx.x;
+    long long w = a.item0 + blockIdx.x;
     if (w >= a.nitems) return;
     unsigned* done_count = reinterpret_cast<unsigned*>(smem + 64);  // [2]: warps that finished the hop phase of even / odd items
     if (threadIdx.x == 0) {
