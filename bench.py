@@ -725,7 +725,7 @@ def main():
                        "parallelism": "replicas" if world > 1 else "single GPU"},
             "clocks": clocks, "gpu_launches": int(launches),
             "e2e": {"value": round(e2e_val, 2), "unit": "GFlop/s", "h2d_bytes_per_step": fb, "d2h_bytes_per_step": fb,
-                    "call": "dwf_apply_host(DWF_DDW, nrhs=1): pinned host canonical in -> H2D -> import -> D_DW -> export -> D2H",
+                    "call": "dwf_apply_host(DWF_DDW, nrhs=1): pinned host canonical in -> H2D -> import -> D_DW -> export -> D2H, pipelined over 16 chunks of t-slices (both copy directions at once)",
                     "ms": round(e2e_s * 1e3, 3)},
             "roofline": roofline, "detail": detail}
     if not args.no_extras and world == 1:
