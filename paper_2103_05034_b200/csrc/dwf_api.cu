@@ -43,6 +43,7 @@ struct dwf_ctx {
     double* scal_host;    // pinned mirror
     int sm_count, device;
     size_t l2_bytes;      // cudaDevAttrL2CacheSize (picks the t-extent of the lattice blocks, build_tables)
+    bool no_dyn;          // DWF_NO_DYN: static instead of dynamic item assignment in the tiled stencil
     bool no_fuse_moo, no_fuse_norm;   // DWF_NO_FUSE_MOOINV / DWF_NO_FUSE_NORM, read once at dwf_create (the unfused reference path)
     int cg_graph;         // DWF_CG_GRAPH, read once at dwf_create: 0 never, 1 always, unset (-1): launch-bound sizes only
     // the instantiated CUDA graph of the last CG solve and the arguments it was captured for (re-launched when they recur)
@@ -224,6 +225,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
     { int l2 = 0; if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev) != cudaSuccess || l2 <= 0) l2 = 64 << 20; h->l2_bytes = (size_t)l2; }
     h->no_fuse_moo = getenv("DWF_NO_FUSE_MOOINV") != nullptr;
     h->no_fuse_norm = getenv("DWF_NO_FUSE_NORM") != nullptr;
+    h->no_dyn = getenv("DWF_NO_DYN") != nullptr;
     { const char* genv = getenv("DWF_CG_GRAPH"); h->cg_graph = genv ? atoi(genv) : -1; }
     std::vector<int> lex, nbr;
     build_tables(h, lex, nbr);
@@ -419,6 +421,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.glinks[1] = (const R*)((const char*)h->glinks + (size_t)h->V4h * lsite);
     a.sigma = (R)(-2.0 * k.c_hop);                                             // links carry the factor -1/2
     a.norm_partial = h->partial; a.norm_out = k.norm_out; a.ticket = h->ticket;
+    a.dyn_counter = h->no_dyn ? nullptr : h->ticket + 2;
     a.ax_num = k.ax_num; a.ax_den = k.ax_den;
     {
         const double kappa = 1.0 / (5.0 - h->M5);

@@ -42,6 +42,7 @@ template <typename R> struct HopArgs {
     const R* glinks[2];    // [p] gathered links of parity-p sites: [site][mu][fwd 18 | bwd 18] x (-1/2), 16 B pad per site
     R sigma;               // res = sigma * hop' + self  with hop' built from the (-1/2)-scaled links
     R moo_kappa, moo_v0scale;   // fused M_oo^-1 epilogue: 1/(5-M5), kappa / (1 + m kappa^Ls)
+    unsigned* dyn_counter; // tiled kernel, non-NORM variants: [0] items handed out beyond the first two rounds, [1] CTAs that left (NULL: static assignment)
     long long item0;       // this launch covers work items item0 .. nitems-1 (a partial launch covers whole lattice blocks)
     long long nitems;      // end of the work items (tile | site group, rhs, parity slot) of this launch
     double* norm_partial;  // NORM epilogue: |out|^2 partials [CTA][warp][2] (each warp's running sum over its items, in item order)

@@ -157,13 +157,23 @@ hop_tile_kernel(const HopArgs<R> a) {
         bulk_g2s(smem + 128 + ib * TG::INT_STRIDE, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int + ib);
     };
 
+    // Which items does this CTA work on?  NORM variants (per-warp running sums must not depend on timing): item0 + blockIdx.x + i gridDim.x.
+    // All others: the first two items are static, every further one is taken from a global counter when the CTA gets there, two
+    // items ahead of its use (DYN).  Fast CTAs then take more items and the items in flight stay one contiguous window of the
+    // sweep; with the static assignment the CTAs drift apart over the rounds of a launch and the window -- the L2 footprint --
+    // widens.  The result of an item does not depend on who computes it.
+    constexpr bool DYN = (NSTI == 1) && !NORM;
+    volatile unsigned* q_item = reinterpret_cast<volatile unsigned*>(smem + 96);   // [4]: item of this CTA's sequence number it, at slot it & 3
+    volatile int* q_seq = reinterpret_cast<volatile int*>(smem + 112);             // highest sequence number whose slot is filled
+    const bool dyn = DYN && a.dyn_counter != nullptr;
     long long w = a.item0 + blockIdx.x;
-    if (w >= a.nitems) return;
+    if (w >= a.nitems) return;                                 // the host never launches more CTAs than items
     unsigned* done_count = reinterpret_cast<unsigned*>(smem + 64);  // [2]: warps that finished the hop phase of even / odd items
     if (threadIdx.x == 0) {
         mbar_init(bar_int, 1); mbar_init(bar_int + 1, 1); mbar_init(bar_small, 1); mbar_init(bar_small + 1, 1);
         mbar_fence_init();
         done_count[0] = 0; done_count[1] = 0;
+        q_item[0] = (unsigned)w; q_item[1] = (unsigned)(w + gridDim.x < a.nitems ? w + gridDim.x : a.nitems); *q_seq = 1;
         issue_small(w, 0); issue_interior(w, 0);
         if (w + gridDim.x < a.nitems) { issue_small(w + gridDim.x, 1); if (NSTI == 2) issue_interior(w + gridDim.x, 1); }
     }
@@ -178,10 +188,15 @@ hop_tile_kernel(const HopArgs<R> a) {
     if constexpr (AXPBY) {
         if (a.ax_num) { const double den = *a.ax_den; ax_a = den != 0.0 ? (R)(-(*a.ax_num / den)) : R(0); }
     }
-    for (int it = 0; w < a.nitems; it++, w += gridDim.x) {
+    for (int it = 0; ; it++) {
+        if (it > 0) {
+            if constexpr (DYN) { while (*q_seq < it) __nanosleep(20); w = q_item[it & 3]; }
+            else w += gridDim.x;
+        }
+        if (w >= a.nitems) break;
         long long gg; int r, pi;
         decode(w, gg, r, pi);
-        const long long wn = w + gridDim.x;
+        const long long wn = w + gridDim.x;                    // static assignment only
         const int buf = it & 1;
         const long long site = gg * TS + ls;
         const long long blk = blk_index(site, r, a.nrhs, SH);
@@ -234,8 +249,19 @@ hop_tile_kernel(const HopArgs<R> a) {
                     if (prev == (unsigned)((it >> 1) + 1) * NWARPS - 1) {
                         // generic-proxy accesses of the buffers (reads; the MOO transpose also writes) before the async-proxy refill
                         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                        if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);
-                        if (wn + gridDim.x < a.nitems) { issue_small(wn + gridDim.x, buf); if (NSTI == 2) issue_interior(wn + gridDim.x, buf); }
+                        if constexpr (DYN) {
+                            const long long w1 = q_item[(it + 1) & 3];             // filled one refill ago (or at the start)
+                            if (w1 < a.nitems) issue_interior(w1, 0);
+                            long long w2 = a.nitems;
+                            if (w1 < a.nitems) w2 = dyn ? a.item0 + 2LL * gridDim.x + atomicAdd(a.dyn_counter, 1u) : w1 + gridDim.x;
+                            q_item[(it + 2) & 3] = (unsigned)(w2 < a.nitems ? w2 : a.nitems);
+                            __threadfence_block();
+                            *q_seq = it + 2;
+                            if (w2 < a.nitems) issue_small(w2, buf);
+                        } else {
+                            if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);
+                            if (wn + gridDim.x < a.nitems) { issue_small(wn + gridDim.x, buf); if (NSTI == 2) issue_interior(wn + gridDim.x, buf); }
+                        }
                     }
                 }
             };
@@ -344,6 +370,13 @@ hop_tile_kernel(const HopArgs<R> a) {
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) sre += __shfl_xor_sync(0xffffffffu, sre, off);
             norm_run += sre;
+        }
+    }
+    if (dyn) {                                                 // the last CTA to leave zeroes the item counter for the next launch
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            if (atomicAdd(a.dyn_counter + 1, 1u) == gridDim.x - 1) { a.dyn_counter[0] = 0u; a.dyn_counter[1] = 0u; __threadfence(); }
         }
     }
     if constexpr (NORM) {
