@@ -55,6 +55,7 @@ struct dwf_ctx {
     cudaEvent_t io_ev[2 * 16 + 1];       //   chunk c arrived / chunk c exported / the handle's stream reached the call
     int tile_sites;       // sites per parity in one tile of the native site order (0: lattice is not made of whole tiles)
     int sg_shift;         // block order [site group][rhs][site in group]: log2(group size)
+    bool rhs_batch;       // one rhs-major stencil launch for a batch of right-hand sides (off: DWF_RHS_LOOP=1 or static item assignment)
     int rhs_chunk;        // right-hand sides per stencil launch
     long long launches;
     char err[256];
@@ -108,9 +109,11 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     // block 4,4,4,2 against 4,4,4,4: D_DW fp32 130.5 -> 127.0 us, fp64 304 -> 281 us, H_DW fp64 nrhs 12 3.81 -> 3.67 ms.  When a layer is
     // far larger than L2 (48^3x96x24: 510 MB) every t face misses anyway and the taller block halves the faces: 4,4,4,4 21.4 ms,
     // 4,4,4,2 25.1 ms, 4,4,4,8 23.7 ms (larger blocks lengthen the y/z reuse distance instead).
+    bool big_layers;
     {
         const double layer2 = (double)L[0] * L[1] * L[2] * 2 * ((double)h->Ls * 24 * 2 + 2 * 72) * real_bytes(h);
-        if (2 * layer2 <= (double)h->l2_bytes) B[3] = 2;
+        big_layers = 2 * layer2 > (double)h->l2_bytes;
+        if (!big_layers) B[3] = 2;
     }
     auto parse = [](const char* name, int* v) {
         if (const char* env = getenv(name)) { int b[4]; if (sscanf(env, "%d,%d,%d,%d", &b[0], &b[1], &b[2], &b[3]) == 4) for (int i = 0; i < 4; i++) v[i] = b[i]; }
@@ -122,7 +125,7 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
     if ((T[0] * T[1] * T[2] * T[3]) % 2 != 0) for (int i = 0; i < 4; i++) T[i] = B[i];
     const long long V4 = h->V4, V4h = h->V4h;
     h->blk_sites = (long long)B[0] * B[1] * B[2] * B[3] / 2;
-    h->blk_t = (getenv("DWF_BLOCK_ORDER") == nullptr && L[3] % B[3] == 0) ? B[3] : 0;   // lexicographic block order: t-layers of blocks are contiguous site ranges
+    { const char* o = getenv("DWF_BLOCK_ORDER"); const bool lexo = o ? !strcmp(o, "lex") : !big_layers; h->blk_t = (lexo && L[3] % B[3] == 0) ? B[3] : 0; }   // lexicographic block order: t-layers of blocks are contiguous site ranges
     const int tsites = T[0] * T[1] * T[2] * T[3] / 2;
     bool whole = true;
     for (int i = 0; i < 4; i++) whole = whole && (L[i] % T[i] == 0);
@@ -144,8 +147,14 @@ static void build_tables(dwf_ctx* h, std::vector<int>& lex, std::vector<int>& nb
         blocks.push_back({bx, by, bz, bt});
     {
         const char* ord = getenv("DWF_BLOCK_ORDER");
+        // Lattices whose t-layers are far larger than L2 (48^3x96x24: 510 MB): panels (the (x,y,z) cross-section cut so that a panel's
+        // layer fits half the L2, t swept inside each panel) keep the z and t halos resident.  Measured on B200 with the dynamic item
+        // assignment of the tiled kernel: D_DW 19.1 ms lexicographic, 18.3-18.7 ms panels of 16-128 MB, 18.4 ms Morton.  (With the
+        // static assignment every order but the lexicographic one DOUBLED the DRAM reads: the CTAs drift apart and the window of items
+        // in flight outgrows the L2.)  "lex" forces the lexicographic order.
+        if (!ord && big_layers) ord = "panel";
         const double block_mb = (double)B[0] * B[1] * B[2] * B[3] * ((double)h->Ls * 24 * 2 + 72) * real_bytes(h) / 1e6;   // in + out + links
-        double budget_mb = 80.0;                                // of the 126 MB L2 (DWF_L2_BUDGET_MB overrides: tuning)
+        double budget_mb = (double)h->l2_bytes / 2e6;           // half the L2 (DWF_L2_BUDGET_MB overrides: tuning)
         if (const char* e = getenv("DWF_L2_BUDGET_MB")) budget_mb = std::max(1.0, atof(e));
         if (ord && !strcmp(ord, "morton")) {
             auto code = [](const std::array<int, 4>& b) {
@@ -231,7 +240,8 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
     build_tables(h, lex, nbr);
     h->rhs_chunk = 1;      // measured on B200 (16^3x32x16 fp32): 1 is fastest (132 us per rhs at nrhs 12; 4: 142 us): a chunk of c rhs needs c slabs of the lattice in L2
     if (const char* env = getenv("DWF_RHS_CHUNK")) h->rhs_chunk = std::max(1, atoi(env));
-    h->partial_doubles = (size_t)MAX_RED_BLOCKS * MAX_NRHS * 2;
+    h->rhs_batch = getenv("DWF_RHS_LOOP") == nullptr && !h->no_dyn;
+    h->partial_doubles = std::max((size_t)MAX_RED_BLOCKS * MAX_NRHS * 2, (size_t)(h->V4h * (Ls / vl(h)) / 32 + 64));   // BLAS-1 partials | fused-norm partials
     for (int n = 1; n <= MAX_NRHS; n++) {                    // worst case of blas_blocks(): one unit of blocks larger than MAX_RED_BLOCKS
         const long long unit = blas_unit((long long)run_groups(h) * n);
         h->partial_doubles = std::max(h->partial_doubles, (size_t)blas_blocks_for(unit, MAX_RED_BLOCKS) * n * 2);
@@ -439,6 +449,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
             attr_done |= 1ull << (h->device & 63); \
         } \
         const long long ctas = std::min<long long>(a.nitems - a.item0, (long long)h->sm_count * TG::MIN_CTAS); \
+        if (a.nitems - a.item0 <= 2 * ctas) a.dyn_counter = nullptr;   /* launch-bound sizes: nothing to hand out, skip the counter traffic */ \
         kern<<<(unsigned)ctas, TG::THREADS, TG::SMEM_BYTES, st>>>(a); } while (0)
 #define HOPM(LS) \
     switch (k.mode) { \
@@ -464,7 +475,13 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     if ((k.norm_out || k.mode == HM_HOP_SELF_AXPBY_NORM) && (!TS || k.nrhs != 1)) FAIL(h, DWF_EINVAL, "fused norm needs the tiled kernel and nrhs = 1");
     // Right-hand sides are processed in chunks (one launch each) so that the working set of a chunk keeps
     // the L2 reuse of the single-rhs case; CTAs of one chunk run tile-major, rhs-minor.
-    const int RC = h->rhs_chunk;
+    // Default (rhs_chunk 1): ONE launch for the whole batch with the items ordered rhs-major -- every rhs sweeps the lattice on its own
+    // (DESIGN.md sec. 5.3), without the ramp-up, the partly filled last round and the launch gap of one launch per rhs.  It needs the
+    // dynamic item assignment of the tiled kernel: with the static one the CTAs drift apart over the 330 rounds of a 24-rhs launch
+    // and it is 15 % SLOWER than one launch per rhs.  DWF_RHS_LOOP=1: one launch per rhs; DWF_RHS_CHUNK=c > 1: tile-major chunks of c rhs.
+    const bool batch = TS && h->rhs_chunk == 1 && h->rhs_batch && k.nrhs > 1 && !k.site1 && !k.norm_out && groups * k.nrhs < (1LL << 31);
+    const int RC = batch ? k.nrhs : h->rhs_chunk;
+    a.items_per_rhs = batch ? (unsigned)groups : 0u;
     for (int r0 = 0; r0 < k.nrhs; r0 += RC) {
         a.r0 = r0; a.rn = std::min(RC, k.nrhs - r0);
         a.item0 = group0 * a.rn; a.nitems = groups * a.rn;
@@ -533,7 +550,7 @@ static int reduce_to(dwf_ctx* h, bool norm, const void* x, const void* y, int nr
 // Can the |out|^2 of a stencil launch be summed inside the launch (tiled kernel, one rhs, partials fit the scratch)?
 static bool norm_fusable(const dwf_ctx* h, int nrhs) {
     return tiled_ok(h) && !h->no_fuse_moo && !h->no_fuse_norm && nrhs == 1
-        && (size_t)h->sm_count * 4 * 32 * 2 <= h->partial_doubles;              // <= 4 CTAs per SM, <= 32 warps per CTA
+        && (size_t)(h->V4h * (h->Ls / vl(h)) / 32) <= h->partial_doubles;       // one partial per (tile, warp) of a half-lattice launch
 }
 struct SchurFuse {          // dag only (CG, q = M^dag w): r <- r - (num/den) q instead of storing q, and *norm_out = |r|^2
     void* r; const double* num; const double* den;

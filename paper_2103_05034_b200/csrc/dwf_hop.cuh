@@ -43,6 +43,7 @@ template <typename R> struct HopArgs {
     R sigma;               // res = sigma * hop' + self  with hop' built from the (-1/2)-scaled links
     R moo_kappa, moo_v0scale;   // fused M_oo^-1 epilogue: 1/(5-M5), kappa / (1 + m kappa^Ls)
     unsigned* dyn_counter; // tiled kernel, non-NORM variants: [0] items handed out beyond the first two rounds, [1] CTAs that left (NULL: static assignment)
+    unsigned items_per_rhs; // tiled kernel: != 0: items are ordered rhs-major, this many per right-hand side (0: tile-major, rhs-minor)
     long long item0;       // this launch covers work items item0 .. nitems-1 (a partial launch covers whole lattice blocks)
     long long nitems;      // end of the work items (tile | site group, rhs, parity slot) of this launch
     double* norm_partial;  // NORM epilogue: |out|^2 partials [CTA][warp][2] (each warp's running sum over its items, in item order)

@@ -75,7 +75,8 @@ template <typename R, int LS, int TS> struct TileGeom {
     // has the SM to itself (384 threads: fp32 Ls 24) a second buffer was measured SLOWER on B200 (48^3x96x24 D_DW 28.3 ms
     // against 21.0 ms): the 72 KB it takes away from L1 cost more (halo and s+-1 loads hit L1) than the exposed refill.
     static constexpr int NSTI = DWF_INT_STAGES;
-    static constexpr unsigned SMEM_BYTES = 128 + NSTI * INT_STRIDE + 2 * SMALL_BYTES;
+    static constexpr unsigned HDR = 256;     // mbarriers, counters, the queue of decoded work items
+    static constexpr unsigned SMEM_BYTES = HDR + NSTI * INT_STRIDE + 2 * SMALL_BYTES;
 };
 
 // load the 18 reals of one link from the gathered shared-memory layout; HALF = 0: U_mu(x), 1: U_mu(x-mu)
@@ -127,13 +128,19 @@ hop_tile_kernel(const HopArgs<R> a) {
     constexpr int NSTI = TG::NSTI;
     unsigned long long* bar_int = reinterpret_cast<unsigned long long*>(smem);          // [NSTI]: interior landed
     unsigned long long* bar_small = reinterpret_cast<unsigned long long*>(smem) + 2;    // [2]: links + nbr landed
-    unsigned char* s_small = smem + 128 + NSTI * TG::INT_STRIDE;
+    unsigned char* s_small = smem + TG::HDR + NSTI * TG::INT_STRIDE;
 
     // work item w -> (tile gg, rhs r, parity slot pi): same order as the CTAs of the generic kernel
     const unsigned rn = (unsigned)a.rn, cg = (unsigned)a.chunk_groups;     // item counts fit 32 bits (checked by the host)
     auto decode = [&](long long w, long long& gg_out, int& r, int& pi) {
-        unsigned gg = (unsigned)w / rn;
-        r = a.r0 + (int)((unsigned)w - gg * rn);
+        unsigned gg;
+        if (a.items_per_rhs) {                                 // rhs-major: all items of one right-hand side, then the next (one launch for the batch)
+            const unsigned ri = (unsigned)w / a.items_per_rhs;
+            gg = (unsigned)w - ri * a.items_per_rhs; r = a.r0 + (int)ri;
+        } else {
+            gg = (unsigned)w / rn;
+            r = a.r0 + (int)((unsigned)w - gg * rn);
+        }
         pi = 0;
         if (a.nslots == 2) {
             const unsigned q = gg / (2 * cg);
@@ -143,28 +150,36 @@ hop_tile_kernel(const HopArgs<R> a) {
         }
         gg_out = gg;
     };
-    auto issue_small = [&](long long w, int buf) {             // thread 0 only
-        long long gg; int r, pi; decode(w, gg, r, pi);
+    auto issue_small_d = [&](long long gg, int pi, int buf) {  // one thread only
         const int p = (a.parity0 + pi) & 1;
         unsigned char* dst = s_small + buf * TG::SMALL_BYTES;
         mbar_expect_tx(bar_small + buf, TG::SMALL_BYTES);
         bulk_g2s(dst, a.glinks[p] + (size_t)gg * TS * LSITE, TG::LINK_BYTES, bar_small + buf);
         bulk_g2s(dst + TG::LINK_BYTES, a.nbr[pi] + (size_t)gg * TS * 8, TG::NBR_BYTES, bar_small + buf);
     };
-    auto issue_interior = [&](long long w, int ib) {           // thread 0 only
-        long long gg; int r, pi; decode(w, gg, r, pi);
+    auto issue_interior_d = [&](long long gg, int r, int pi, int ib) {   // one thread only
         mbar_expect_tx(bar_int + ib, TG::INTERIOR_BYTES);
-        bulk_g2s(smem + 128 + ib * TG::INT_STRIDE, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int + ib);
+        bulk_g2s(smem + TG::HDR + ib * TG::INT_STRIDE, a.in_hop[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS, TG::INTERIOR_BYTES, bar_int + ib);
     };
+    auto issue_small = [&](long long w, int buf) { long long gg; int r, pi; decode(w, gg, r, pi); issue_small_d(gg, pi, buf); };
+    auto issue_interior = [&](long long w, int ib) { long long gg; int r, pi; decode(w, gg, r, pi); issue_interior_d(gg, r, pi, ib); };
 
-    // Which items does this CTA work on?  NORM variants (per-warp running sums must not depend on timing): item0 + blockIdx.x + i gridDim.x.
-    // All others: the first two items are static, every further one is taken from a global counter when the CTA gets there, two
-    // items ahead of its use (DYN).  Fast CTAs then take more items and the items in flight stay one contiguous window of the
-    // sweep; with the static assignment the CTAs drift apart over the rounds of a launch and the window -- the L2 footprint --
-    // widens.  The result of an item does not depend on who computes it.
-    constexpr bool DYN = (NSTI == 1) && !NORM;
-    volatile unsigned* q_item = reinterpret_cast<volatile unsigned*>(smem + 96);   // [4]: item of this CTA's sequence number it, at slot it & 3
+    // Which items does this CTA work on?  The first two are static (item0 + blockIdx.x, + gridDim.x), every further one is taken
+    // from a global counter when the CTA gets there, two items ahead of its use (DYN).  Fast CTAs then take more items and the
+    // items in flight stay one contiguous window of the sweep; with a static round-robin assignment the CTAs drift apart over the
+    // rounds of a launch and the window -- the L2 footprint -- widens.  No result depends on who computes an item: the NORM
+    // epilogue keeps one partial per (item, warp), summed in index order.
+    constexpr bool DYN = (NSTI == 1);
+    // the queue: slot it & 3 holds the decoded item of this CTA's sequence number it, {item, tile, rhs, parity slot}; item = nitems: none.
+    // Only the refilling thread decodes (two integer divisions); the other threads read the slot.
+    volatile int4* q_slot = reinterpret_cast<volatile int4*>(smem + 128);          // [4]
     volatile int* q_seq = reinterpret_cast<volatile int*>(smem + 112);             // highest sequence number whose slot is filled
+    auto q_put = [&](int seq, long long w) -> bool {           // one thread only; returns whether there is such an item
+        int4 v = make_int4((int)a.nitems, 0, 0, 0);
+        if (w < a.nitems) { long long gg; int r, pi; decode(w, gg, r, pi); v = make_int4((int)w, (int)gg, r, pi); }
+        q_slot[seq & 3].x = v.x; q_slot[seq & 3].y = v.y; q_slot[seq & 3].z = v.z; q_slot[seq & 3].w = v.w;
+        return w < a.nitems;
+    };
     const bool dyn = DYN && a.dyn_counter != nullptr;
     long long w = a.item0 + blockIdx.x;
     if (w >= a.nitems) return;                                 // the host never launches more CTAs than items
@@ -173,9 +188,11 @@ hop_tile_kernel(const HopArgs<R> a) {
         mbar_init(bar_int, 1); mbar_init(bar_int + 1, 1); mbar_init(bar_small, 1); mbar_init(bar_small + 1, 1);
         mbar_fence_init();
         done_count[0] = 0; done_count[1] = 0;
-        q_item[0] = (unsigned)w; q_item[1] = (unsigned)(w + gridDim.x < a.nitems ? w + gridDim.x : a.nitems); *q_seq = 1;
-        issue_small(w, 0); issue_interior(w, 0);
-        if (w + gridDim.x < a.nitems) { issue_small(w + gridDim.x, 1); if (NSTI == 2) issue_interior(w + gridDim.x, 1); }
+        { long long gg; int r, pi; decode(w, gg, r, pi);       // decode once, copies first
+          issue_small_d(gg, pi, 0); issue_interior_d(gg, r, pi, 0);
+          q_slot[0].x = (int)w; q_slot[0].y = (int)gg; q_slot[0].z = r; q_slot[0].w = pi; }
+        if (q_put(1, w + gridDim.x)) { issue_small_d(q_slot[1].y, q_slot[1].w, 1); if (NSTI == 2) issue_interior_d(q_slot[1].y, q_slot[1].z, q_slot[1].w, 1); }
+        *q_seq = 1;
     }
     __syncthreads();
     constexpr unsigned NWARPS = TG::THREADS / 32;
@@ -183,19 +200,22 @@ hop_tile_kernel(const HopArgs<R> a) {
     const int ls = threadIdx.x / K;                            // site within the tile
     const int k = threadIdx.x - ls * K;
 
-    double norm_run = 0.0;                                     // NORM: this warp's running |out|^2 (lane 0), items in launch order
     R ax_a = a.ax_a;
     if constexpr (AXPBY) {
         if (a.ax_num) { const double den = *a.ax_den; ax_a = den != 0.0 ? (R)(-(*a.ax_num / den)) : R(0); }
     }
     for (int it = 0; ; it++) {
-        if (it > 0) {
-            if constexpr (DYN) { while (*q_seq < it) __nanosleep(20); w = q_item[it & 3]; }
-            else w += gridDim.x;
-        }
-        if (w >= a.nitems) break;
         long long gg; int r, pi;
-        decode(w, gg, r, pi);
+        if constexpr (DYN) {
+            while (*q_seq < it) __nanosleep(20);
+            const volatile int4* sl = q_slot + (it & 3);
+            w = sl->x; gg = sl->y; r = sl->z; pi = sl->w;
+            if (w >= a.nitems) break;
+        } else {
+            if (it > 0) w += gridDim.x;
+            if (w >= a.nitems) break;
+            decode(w, gg, r, pi);
+        }
         const long long wn = w + gridDim.x;                    // static assignment only
         const int buf = it & 1;
         const long long site = gg * TS + ls;
@@ -220,7 +240,7 @@ hop_tile_kernel(const HopArgs<R> a) {
             const int4 n0 = nb4[0], n1 = nb4[1];
             const R* u = reinterpret_cast<const R*>(small) + ls * LSITE;
             const int ib = (NSTI == 2) ? buf : 0;
-            const G* s_in = reinterpret_cast<const G*>(smem + 128 + ib * TG::INT_STRIDE);
+            const G* s_in = reinterpret_cast<const G*>(smem + TG::HDR + ib * TG::INT_STRIDE);
             const G* in = a.in_hop[pi] + k;
             // neighbour block: inside the tile -> shared memory, else global memory
             auto nb = [&](int n) -> const G* {
@@ -250,14 +270,15 @@ hop_tile_kernel(const HopArgs<R> a) {
                         // generic-proxy accesses of the buffers (reads; the MOO transpose also writes) before the async-proxy refill
                         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
                         if constexpr (DYN) {
-                            const long long w1 = q_item[(it + 1) & 3];             // filled one refill ago (or at the start)
-                            if (w1 < a.nitems) issue_interior(w1, 0);
+                            const volatile int4* s1 = q_slot + ((it + 1) & 3);     // filled one refill ago (or at the start)
+                            const bool have1 = s1->x < (int)a.nitems;
+                            if (have1) issue_interior_d(s1->y, s1->z, s1->w, 0);
                             long long w2 = a.nitems;
-                            if (w1 < a.nitems) w2 = dyn ? a.item0 + 2LL * gridDim.x + atomicAdd(a.dyn_counter, 1u) : w1 + gridDim.x;
-                            q_item[(it + 2) & 3] = (unsigned)(w2 < a.nitems ? w2 : a.nitems);
+                            if (have1) w2 = dyn ? a.item0 + 2LL * gridDim.x + atomicAdd(a.dyn_counter, 1u) : (long long)s1->x + gridDim.x;
+                            const bool have2 = q_put(it + 2, w2);
                             __threadfence_block();
                             *q_seq = it + 2;
-                            if (w2 < a.nitems) issue_small(w2, buf);
+                            if (have2) { const volatile int4* s2 = q_slot + ((it + 2) & 3); issue_small_d(s2->y, s2->w, buf); }
                         } else {
                             if (NSTI == 1 && wn < a.nitems) issue_interior(wn, 0);
                             if (wn + gridDim.x < a.nitems) { issue_small(wn + gridDim.x, buf); if (NSTI == 2) issue_interior(wn + gridDim.x, buf); }
@@ -275,7 +296,7 @@ hop_tile_kernel(const HopArgs<R> a) {
                 // interior buffer (rows = (site, component), padded by one group against bank conflicts), then one
                 // thread per row walks s in registers and stores the row (contiguous in the output block).
                 constexpr int VL = Prec<R>::VL;
-                G* s_t = reinterpret_cast<G*>(smem + 128 + ib * TG::INT_STRIDE);    // this item's interior buffer
+                G* s_t = reinterpret_cast<G*>(smem + TG::HDR + ib * TG::INT_STRIDE);    // this item's interior buffer
                 __syncthreads();                               // every warp is done reading the interior
 #pragma unroll
                 for (int c = 0; c < 12; c++) s_t[(ls * 12 + c) * (K + 1) + k] = pack(acc[c]);
@@ -362,14 +383,13 @@ hop_tile_kernel(const HopArgs<R> a) {
 #pragma unroll
         for (int c = 0; c < 12; c++) __stcs(o + c * K, pack(acc[c]));          // streaming store: the output is not re-read by this launch
         if constexpr (NORM) {
-            // |out|^2 of this item, fp64: fixed shuffle tree inside the warp, added to the warp's running sum.  The items of a
-            // CTA are a fixed function of the launch geometry, so the result does not depend on the timing of the CTAs.
+            // |out|^2 of this warp's part of the item, fp64: fixed shuffle tree inside the warp, one partial per (item, warp)
             double sre = 0, sim = 0;
 #pragma unroll
             for (int c = 0; c < 12; c++) acc_inner(sre, sim, acc[c], acc[c]);
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) sre += __shfl_xor_sync(0xffffffffu, sre, off);
-            norm_run += sre;
+            if ((threadIdx.x & 31) == 0) a.norm_partial[(size_t)(w - a.item0) * NWARPS + (threadIdx.x >> 5)] = sre;
         }
     }
     if (dyn) {                                                 // the last CTA to leave zeroes the item counter for the next launch
@@ -380,12 +400,8 @@ hop_tile_kernel(const HopArgs<R> a) {
         }
     }
     if constexpr (NORM) {
-        // one partial per (CTA, warp); the last CTA to arrive sums them in (CTA, warp) order: deterministic, no extra launch
+        // the last CTA to arrive sums the (item, warp) partials in index order: deterministic, no extra launch
         __shared__ bool s_last;
-        if ((threadIdx.x & 31) == 0) {
-            double* slot = a.norm_partial + ((size_t)blockIdx.x * NWARPS + (threadIdx.x >> 5)) * 2;
-            slot[0] = norm_run; slot[1] = 0.0;
-        }
         __threadfence();
         __syncthreads();
         if (threadIdx.x == 0) s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1);
@@ -393,9 +409,14 @@ hop_tile_kernel(const HopArgs<R> a) {
         if (s_last) {
             __threadfence();
             __shared__ double s_sum[TG::THREADS];
-            const int n = (int)(gridDim.x * NWARPS);
+            // NWARPS is even and the slots are 16-byte aligned: 128-bit loads, 16 in flight per thread (the sum is one L2 round trip or
+            // two at 16^3x32: 16k partials; fixed order per thread, then thread order)
+            static_assert(NWARPS % 2 == 0, "pairs of partials");
+            const long long n2 = (a.nitems - a.item0) * (NWARPS / 2);
+            const double2* pp = reinterpret_cast<const double2*>(a.norm_partial);
             double t = 0;
-            for (int k = threadIdx.x; k < n; k += TG::THREADS) t += __ldcg(a.norm_partial + (size_t)k * 2);
+#pragma unroll 16
+            for (long long k = threadIdx.x; k < n2; k += TG::THREADS) { const double2 v = __ldcg(pp + k); t += v.x; t += v.y; }
             s_sum[threadIdx.x] = t;
             __syncthreads();
             if (threadIdx.x == 0) {
