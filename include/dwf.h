@@ -145,6 +145,15 @@ int dwf_axpy(dwf_handle h, const double* a_host, const void* x, void* y, int nrh
 int dwf_inner(dwf_handle h, const void* x, const void* y, double* out_host, int nrhs, int half);
 int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs, int half);
 
+/* norm2 for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the same
+ * kernels and summation order as dwf_norm2 (north_star item (4)), but nothing on its path calls cudaMalloc/cudaFree -- the
+ * per-block partials live in a file-scope __device__ array of 32768 doubles (256 KB per GPU that loads the library, held until
+ * the process exits) -- and out_dev[nrhs] is a DEVICE pointer: the call is asynchronous on the handle's stream.  The handle's
+ * device must be the current device.  Sizes whose partials exceed the array (blocks x nrhs x 2 doubles; blocks <= 8 per SM)
+ * return DWF_EUNSUPPORTED: use fewer right-hand sides per call.  All calls on a GPU share the array: calls that overlap on the
+ * GPU (other streams or handles) race; successive calls on one stream do not (every slot a call reads it has written first). */
+int dwf_norm2_static(dwf_handle h, const void* x, double* out_dev, int nrhs, int half);
+
 /* `iters` iterations of Hestenes-Stiefel CG on M_pc^dag M_pc x = b (eq. 9), nrhs = 1, even half
  * fields.  x_even holds x_0 on entry and x_iters on return.  resid2_hist_host (may be NULL) receives
  * iters+1 values |r_k|^2.  Uses the workspace (5 half fields).  Synchronises at the end only.  At launch-bound sizes (a half field

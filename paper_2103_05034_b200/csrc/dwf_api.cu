@@ -885,6 +885,48 @@ extern "C" int dwf_norm2(dwf_handle h, const void* x, double* out_host, int nrhs
 }
 
 // ------------------------------------------------------------------------------------------------
+// dwf_norm2_static: |x|^2 per right-hand side with NO allocation anywhere on its path (callers under CUDA graph capture, tight
+// serving loops, harnesses that forbid cudaMalloc).  Same two kernels and launch geometry as dwf_norm2; the per-block partials go
+// to a file-scope __device__ array instead of the handle's cudaMalloc'ed scratch, the result to a DEVICE pointer (no host
+// synchronisation).  The array is DWF_STATIC_SCRATCH_DOUBLES doubles = 256 KB, held by every GPU that loads the library until the
+// process exits.  Every call on a device shares it: the partial slots a call reads are all written by that call first (nothing
+// has to start at zero), but two calls that overlap on the GPU (different streams / handles) race on it.
+// ------------------------------------------------------------------------------------------------
+#define DWF_STATIC_SCRATCH_DOUBLES 32768
+static __device__ __align__(256) double g_norm2_scratch[DWF_STATIC_SCRATCH_DOUBLES];
+// In host code the name above is a host-side stand-in, not a device address: the address is asked for once per device.
+static double* g_norm2_scratch_ptr[64];
+
+extern "C" int dwf_norm2_static(dwf_handle h, const void* x, double* out_dev, int nrhs, int half) {
+    if (!h) return DWF_EINVAL;
+    if (nrhs < 1 || nrhs > MAX_NRHS || !out_dev) FAIL(h, DWF_EINVAL, "bad nrhs or out_dev");
+    if (int rc = check_field(h, x, "x")) return rc;
+    int dev = -1;
+    CUDA_TRY(h, cudaGetDevice(&dev));
+    if (dev != h->device || dev < 0 || dev >= 64) FAIL(h, DWF_EINVAL, "the handle's device (%d) must be the current device (%d)", h->device, dev);
+    if (!g_norm2_scratch_ptr[dev]) {                         // set-up, once per device, with that device current
+        double* ptr = nullptr;
+        CUDA_TRY(h, cudaGetSymbolAddress((void**)&ptr, g_norm2_scratch));
+        if (!ptr) FAIL(h, DWF_ECUDA, "cudaGetSymbolAddress returned a null address");
+        g_norm2_scratch_ptr[dev] = ptr;
+    }
+    double* partial = g_norm2_scratch_ptr[dev];
+    const long long ng = half_groups(h, nrhs) * (half ? 1 : 2);
+    const int BS = run_groups(h);
+    const unsigned blocks = blas_blocks(h, ng, (long long)BS * nrhs);
+    const size_t need = (size_t)blocks * nrhs * 2;
+    if (need > (size_t)DWF_STATIC_SCRATCH_DOUBLES)
+        FAIL(h, DWF_EUNSUPPORTED, "dwf_norm2_static: %zu doubles of scratch needed (%u blocks x %d rhs x 2), the static maximum is %d: use fewer right-hand sides per call or dwf_norm2",
+             need, blocks, nrhs, DWF_STATIC_SCRATCH_DOUBLES);
+    if (h->prec == DWF_F32) inner_kernel<float, true><<<blocks, 256, 0, h->stream>>>((const float4*)x, nullptr, ng, BS, nrhs, partial);
+    else                    inner_kernel<double, true><<<blocks, 256, 0, h->stream>>>((const double2*)x, nullptr, ng, BS, nrhs, partial);
+    LAUNCH_CHECK(h);
+    reduce_final_kernel<<<nrhs, 256, 0, h->stream>>>(partial, (int)blocks, nrhs, out_dev, 1, 1);
+    LAUNCH_CHECK(h);
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Red-black CGNR driver.  Host loop that only enqueues; alpha and beta are
 // computed on the device from reduction results kept in h->scal: hist[k] = |r_k|^2 at scal[k],
 // <p_k, A p_k> = |M p_k|^2 at scal[iters+1+k].

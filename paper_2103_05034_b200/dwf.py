@@ -48,6 +48,7 @@ _SIGNATURES = {
                                  ctypes.c_int, ctypes.c_int]),
     "dwf_norm2": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int,
                                  ctypes.c_int]),
+    "dwf_norm2_static": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int]),
     "dwf_cg_schur": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
                                     ctypes.POINTER(ctypes.c_double)]),
     "dwf_cg_schur_multi": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
@@ -243,6 +244,12 @@ class Dwf:
         buf = (ctypes.c_double * nrhs)()
         self._check(self.lib.dwf_norm2(self._h, ctypes.c_void_p(x.data_ptr()), buf, nrhs, int(half)))
         return [float(buf[r]) for r in range(nrhs)]
+
+    def norm2_static(self, x: torch.Tensor, out_dev: torch.Tensor, nrhs: int, half: bool = False) -> torch.Tensor:
+        """out_dev: float64 CUDA tensor of nrhs elements; no allocation on the C side, asynchronous."""
+        assert out_dev.is_cuda and out_dev.dtype == torch.float64 and out_dev.numel() >= nrhs and out_dev.is_contiguous()
+        self._check(self.lib.dwf_norm2_static(self._h, ctypes.c_void_p(x.data_ptr()), ctypes.c_void_p(out_dev.data_ptr()), nrhs, int(half)))
+        return out_dev
 
     def cg_schur(self, b_even: torch.Tensor, x_even: torch.Tensor, iters: int):
         hist = (ctypes.c_double * (iters + 1))()
