@@ -5,6 +5,8 @@ oracle in test_gpu_parity.py / test_gpu_fullsize.py through whichever path is th
   * Schur K1 with the fused M_oo^-1 epilogue vs  separate mooinv_kernel            DWF_NO_FUSE_MOOINV=1
   * CG enqueued on the stream                vs  CG captured into a CUDA graph     DWF_CG_GRAPH=1
   * 16- / 32- / 64-site tiles of the tiled stencil (small lattices default to 16)   DWF_TILE=bx,by,bz,bt
+  * dynamic item assignment                  vs  static round robin                DWF_NO_DYN=1
+  * one rhs-major launch per batch of rhs    vs  one launch per rhs                DWF_RHS_LOOP=1
 """
 import numpy as np
 import pytest
@@ -141,3 +143,41 @@ def test_repeatable_bit_for_bit(monkeypatch, prec, tile):
         rig.d.chebyshev(3, 0.01, 70.0, x, c, nrhs)
         rig.d.apply(DWF_SCHUR_EO, xe, s, nrhs)
         assert torch.equal(y, ref_h) and torch.equal(c, ref_c) and torch.equal(s, ref_s)
+
+
+def test_dynamic_vs_static_assignment_and_batch_vs_loop(monkeypatch):
+    """At a size where the tiled kernel hands items out dynamically (more than two items per CTA), no result may depend on which CTA
+    computed an item or on how the right-hand sides were cut into launches: operators, Chebyshev and the CG history (fused norms:
+    one partial per (item, warp), summed in index order) are bit identical across DWF_NO_DYN / DWF_RHS_LOOP and across repeats."""
+    import torch
+    L, Ls, nrhs = (16, 16, 16, 16), 16, 3
+    res = {}
+    for tag, env in (("default", {}), ("static", {"DWF_NO_DYN": "1"}), ("loop", {"DWF_RHS_LOOP": "1"})):
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        rig = Rig(L, Ls, "f32", 0.01, seed_U=61, ws_nrhs=nrhs)
+        for k in env:
+            monkeypatch.delenv(k)
+        g = torch.Generator(device="cuda"); g.manual_seed(62)
+        x = rig.d.field(nrhs).normal_(generator=g)
+        y, c, se = rig.d.field(nrhs), rig.d.field(nrhs), rig.d.field(nrhs, half=True)
+        l0 = rig.d.launch_count()
+        rig.d.apply(DWF_DDW, x, y, nrhs)
+        n_apply = rig.d.launch_count() - l0
+        rig.d.chebyshev(3, 0.01, 70.0, x, c, nrhs)
+        xe = x[: se.numel()].clone()
+        rig.d.apply(DWF_SCHUR_EO, xe, se, nrhs)
+        b = xe[: xe.numel() // nrhs].clone()
+        hists, sols = [], []
+        for _ in range(3 if tag == "default" else 1):
+            xs = rig.d.field(1, half=True, zero=True)
+            hists.append(rig.d.cg_schur(b, xs, 6)); sols.append(xs)
+        assert all(h == hists[0] for h in hists) and all(bool((s_ == sols[0]).all()) for s_ in sols)
+        res[tag] = (y, c, se, hists[0], sols[0], n_apply)
+    assert res["default"][5] == 1 and res["loop"][5] == nrhs           # one launch for the batch / one per rhs
+    for tag in ("static", "loop"):
+        for a, b_ in zip(res["default"][:3], res[tag][:3]):
+            assert torch.equal(a, b_), tag
+        assert res[tag][3] == res["default"][3] and torch.equal(res[tag][4], res["default"][4]), tag
+    # (the default path is compared with the oracle at this kernel geometry -- 32-site tiles, dynamic assignment, batch launches -- by
+    # tests/test_gpu_fullsize.py)
