@@ -43,6 +43,7 @@ struct dwf_ctx {
     double* scal_host;    // pinned mirror
     int sm_count, device;
     size_t l2_bytes;      // cudaDevAttrL2CacheSize (picks the t-extent of the lattice blocks, build_tables)
+    bool cheb_factored;   // DWF_CHEB_FACTORED: dwf_chebyshev steps as alpha (H - c)(H + c) t instead of the literal alpha H(H t) - beta t
     bool no_dyn;          // DWF_NO_DYN: static instead of dynamic item assignment in the tiled stencil
     bool no_fuse_moo, no_fuse_norm;   // DWF_NO_FUSE_MOOINV / DWF_NO_FUSE_NORM, read once at dwf_create (the unfused reference path)
     int cg_graph;         // DWF_CG_GRAPH, read once at dwf_create: 0 never, 1 always, unset (-1): launch-bound sizes only
@@ -235,6 +236,7 @@ extern "C" int dwf_create(const int L[4], int Ls, double M5, double mass, int pr
     h->no_fuse_moo = getenv("DWF_NO_FUSE_MOOINV") != nullptr;
     h->no_fuse_norm = getenv("DWF_NO_FUSE_NORM") != nullptr;
     h->no_dyn = getenv("DWF_NO_DYN") != nullptr;
+    h->cheb_factored = getenv("DWF_CHEB_FACTORED") != nullptr;
     { const char* genv = getenv("DWF_CG_GRAPH"); h->cg_graph = genv ? atoi(genv) : -1; }
     std::vector<int> lex, nbr;
     build_tables(h, lex, nbr);
@@ -377,6 +379,7 @@ struct HopCall {            // precision-independent description of one launch
                             // inside the launch (dwf_tile.cuh NORM epilogue)
     const double* ax_num; const double* ax_den;   // HM_HOP_SELF_AXPBY_NORM: ax_a = -(*ax_num / *ax_den), read on the device
     long long site0, site1;  // output sites (native order, per parity) of this launch, whole lattice blocks; site1 = 0: all
+    double g5_shift;         // HM_HOP_SELF_G5*: out = (H_DW + g5_shift) in [then the axpby epilogue]
 };
 
 // Is the tiled persistent stencil (dwf_tile.cuh) instantiated for this handle?  Lattice made of whole tiles, Ls 16 (16- or
@@ -409,7 +412,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.V4h = h->V4h; a.Ls = h->Ls; a.nrhs = k.nrhs;
     a.parity0 = k.parity0; a.nslots = k.nslots;
     a.c_hop = (R)k.c_hop; a.c_diag = (R)(5.0 - h->M5); a.mass = (R)k.mass;
-    a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c;
+    a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c; a.g5_shift = (R)k.g5_shift;
     const int K = h->Ls / Prec<R>::VL;
     // tiled persistent stencil (dwf_tile.cuh): lattice made of whole tiles, compile-time Ls, a hop to do
     const int TS = (k.mode != HM_SELF && tiled_ok(h)) ? h->tile_sites : 0;
@@ -527,7 +530,7 @@ static int launch_mooinv(dwf_ctx* h, const void* in, void* out, int nrhs, double
 // full-lattice operator:  out_p = c_hop hop(in_{1-p}) [+ self(in_p)] for both parities, one launch
 static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, const void* in, void* out, int nrhs,
                    double ax_a = 0, const void* y = nullptr, double ax_b = 0, const void* z = nullptr, double ax_c = 0,
-                   long long site0 = 0, long long site1 = 0) {
+                   long long site0 = 0, long long site1 = 0, double g5_shift = 0.0) {
     const size_t hb = half_bytes(h, nrhs);
     HopCall k{};
     k.mode = mode; k.dag = dag; k.nslots = 2; k.parity0 = 0; k.nrhs = nrhs;
@@ -539,7 +542,7 @@ static int full_op(dwf_ctx* h, int mode, bool dag, double c_hop, double mass, co
         k.z[p] = z ? (const char*)z + (size_t)p * hb : nullptr;
     }
     k.c_hop = c_hop; k.mass = mass; k.ax_a = ax_a; k.ax_b = ax_b; k.ax_c = ax_c;
-    k.site0 = site0; k.site1 = site1;
+    k.site0 = site0; k.site1 = site1; k.g5_shift = g5_shift;
     return launch_hop(h, k);
 }
 
@@ -652,6 +655,24 @@ extern "C" int dwf_apply(dwf_handle h, int op, const void* in, void* out, int nr
 // overwrites t_{k-1} in place.  Odd t_k live in buffer A, even ones in B; A/B are chosen so that
 // t_order lands in `out`.
 // ------------------------------------------------------------------------------------------------
+// One step of a recurrence in X = alpha H^2 - beta (H = H_DW), two stencil launches through the scratch field w:
+//     dst = coef (alpha H^2 - beta) tk + cz z            (z may alias dst; cz = 0: no z)
+// Literal form (default; SURVEY 8(a) a8, 6 field passes):   w = H tk ;  dst = coef alpha H w - coef beta tk + cz z.
+// Factored form (DWF_CHEB_FACTORED=1, 5 field passes):  alpha H^2 - beta = alpha (H - c)(H + c),  c = sqrt(beta / alpha)  [H is hermitian
+// and commutes with c]:   w = (H + c) tk ;  dst = coef alpha (H - c) w + cz z.   The shift rides in the G5 epilogue (the input at the output
+// location = another lane group of the block the self term has just read), so the second launch no longer reads tk.  Measured on B200:
+// order-64 Chebyshev on 24 vectors 485 -> 474 ms; error against the oracle 9.0e-6 instead of 3.3e-6 (fp32), 1.3e-14 instead of 2.7e-14 (fp64).
+// Opt-in: the bench line and its roofline keep the literal form that SURVEY's algorithmic byte count (144R per 5D site and order) describes.
+static int x_step(dwf_ctx* h, const void* tk, void* w, void* dst, int nrhs, double coef, double alpha, double beta, const void* z, double cz) {
+    if (h->cheb_factored && beta > 0.0 && alpha > 0.0) {
+        const double c = std::sqrt(beta / alpha);
+        if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, tk, w, nrhs, 0, nullptr, 0, nullptr, 0, 0, 0, +c)) return rc;
+        return full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, coef * alpha, z ? z : tk, 0.0, z ? z : tk, z ? cz : 0.0, 0, 0, -c);
+    }
+    if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, tk, w, nrhs)) return rc;
+    return full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, coef * alpha, tk, -coef * beta, z ? z : tk, z ? cz : 0.0);
+}
+
 extern "C" int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, const void* in, void* out, int nrhs) {
     if (!h) return DWF_EINVAL;
     if (nrhs < 1 || nrhs > MAX_NRHS) FAIL(h, DWF_EINVAL, "nrhs must be in [1,%d]", MAX_NRHS);
@@ -669,13 +690,11 @@ extern "C" int dwf_chebyshev(dwf_handle h, int order, double lo, double hi, cons
     void* B = (order & 1) ? other : out;      // holds t_2, t_4, ...
     const double alpha = 2.0 / (hi - lo), beta = (hi + lo) / (hi - lo);
     // t_1 = alpha H H t_0 - beta t_0
-    if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, in, w, nrhs)) return rc;
-    if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, A, nrhs, alpha, in, -beta, in, 0.0)) return rc;
+    if (int rc = x_step(h, in, w, A, nrhs, 1.0, alpha, beta, nullptr, 0.0)) return rc;
     const void* tkm1 = in; void* tk = A;
     for (int k = 1; k < order; k++) {
         void* dst = (k == 1) ? B : (void*)tkm1;           // t_{k+1} overwrites t_{k-1} (except t_0 = user input)
-        if (int rc = full_op(h, HM_HOP_SELF_G5, false, -0.5, h->mass, tk, w, nrhs)) return rc;
-        if (int rc = full_op(h, HM_HOP_SELF_G5_AXPBY, false, -0.5, h->mass, w, dst, nrhs, 2.0 * alpha, tk, -2.0 * beta, tkm1, -1.0)) return rc;
+        if (int rc = x_step(h, tk, w, dst, nrhs, 2.0, alpha, beta, tkm1, -1.0)) return rc;
         tkm1 = tk; tk = dst;
     }
     return DWF_OK;

@@ -55,6 +55,7 @@ template <typename R> struct HopArgs {
     long long chunk_groups;
     R c_hop, c_diag, mass;
     R ax_a, ax_b, ax_c;
+    R g5_shift;            // G5 epilogue: res = Gamma5 (hop + self) + g5_shift * in   (H_DW + shift; 0: none)
 };
 
 // (U h)_a = sum_b U_ab h_b  (FWD)   or   (U^dag h)_a = sum_b conj(U_ba) h_b  (!FWD)
@@ -309,6 +310,14 @@ hop_kernel(const HopArgs<R> a) {
         for (int c = 0; c < 12; c++) {
             acc[c].re = vswap(acc[c].re); acc[c].im = vswap(acc[c].im);
             if (c >= 6) { acc[c].re = vneg(acc[c].re); acc[c].im = vneg(acc[c].im); }
+        }
+        if (SELF && a.g5_shift != R(0)) {                     // res = (H_DW + shift) in, see dwf_tile.cuh
+            const G* t = a.in_self[pi] + (size_t)blk * BS + ko;
+#pragma unroll
+            for (int c = 0; c < 12; c++) {
+                const CV<V> tt = unpack(ldg_nc(t + c * K));
+                acc[c].re = vfma(a.g5_shift, tt.re, acc[c].re); acc[c].im = vfma(a.g5_shift, tt.im, acc[c].im);
+            }
         }
     }
     const size_t obase = (size_t)blk * BS + ko;

@@ -357,6 +357,16 @@ hop_tile_kernel(const HopArgs<R> a) {
                 acc[c].re = vswap(acc[c].re); acc[c].im = vswap(acc[c].im);
                 if (c >= 6) { acc[c].re = vneg(acc[c].re); acc[c].im = vneg(acc[c].im); }
             }
+            // res = (H_DW + shift) in: the input at the OUTPUT location is lane group K-1-k of this thread's own (site, rhs) block,
+            // the lines the self term has just read (L1 hits).  The factored Chebyshev step of dwf_api.cu x_step uses it.
+            if (SELF && a.g5_shift != R(0)) {
+                const G* t = a.in_self[pi] + (size_t)blk * BS + ko;
+#pragma unroll
+                for (int c = 0; c < 12; c++) {
+                    const CV<V> tt = unpack(ldg_nc(t + c * K));
+                    acc[c].re = vfma(a.g5_shift, tt.re, acc[c].re); acc[c].im = vfma(a.g5_shift, tt.im, acc[c].im);
+                }
+            }
         }
         const size_t obase = (size_t)blk * BS + ko;
         if constexpr (AXPBY) {

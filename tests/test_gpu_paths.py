@@ -7,6 +7,7 @@ oracle in test_gpu_parity.py / test_gpu_fullsize.py through whichever path is th
   * 16- / 32- / 64-site tiles of the tiled stencil (small lattices default to 16)   DWF_TILE=bx,by,bz,bt
   * dynamic item assignment                  vs  static round robin                DWF_NO_DYN=1
   * one rhs-major launch per batch of rhs    vs  one launch per rhs                DWF_RHS_LOOP=1
+  * literal Chebyshev step aH(Ht) - bt       vs  factored a(H - c)(H + c)t         DWF_CHEB_FACTORED=1
 """
 import numpy as np
 import pytest
@@ -181,3 +182,29 @@ def test_dynamic_vs_static_assignment_and_batch_vs_loop(monkeypatch):
         assert res[tag][3] == res["default"][3] and torch.equal(res[tag][4], res["default"][4]), tag
     # (the default path is compared with the oracle at this kernel geometry -- 32-site tiles, dynamic assignment, batch launches -- by
     # tests/test_gpu_fullsize.py)
+
+
+@pytest.mark.parametrize("prec,L,Ls", [("f32", (8, 8, 4, 4), 16), ("f64", (8, 4, 4, 4), 16), ("f32", (6, 4, 4, 4), 8)])
+def test_chebyshev_factored_step(oracle, monkeypatch, prec, L, Ls):
+    """DWF_CHEB_FACTORED=1: alpha H^2 - beta applied as alpha (H - c)(H + c), c = sqrt(beta/alpha), the shift fused into the
+    Gamma5 epilogue (tiled and generic kernel).  Same polynomial: against the oracle at the tolerances of the literal form,
+    and against the literal form itself."""
+    mass, nrhs = 0.01, 2
+    tol = {"f32": 1e-4, "f64": 1e-11}[prec]
+    outs = {}
+    for tag in ("literal", "factored"):
+        if tag == "factored":
+            monkeypatch.setenv("DWF_CHEB_FACTORED", "1")
+        rig = Rig(L, Ls, prec, mass, seed_U=71, ws_nrhs=nrhs)
+        psi = rig.spinor(nrhs, 72)
+        res = []
+        for order in (1, 2, 7, 64):
+            out = rig.d.field(nrhs)
+            rig.d.chebyshev(order, 0.01, 70.0, rig.native(psi), out, nrhs)
+            res.append(rig.canonical(out, nrhs))
+        outs[tag] = res
+    for order, a, b in zip((1, 2, 7, 64), outs["literal"], outs["factored"]):
+        want = oracle.chebyshev(rig.U, psi, M5, mass, order, 0.01, 70.0)
+        assert rel_l2(b, want) < tol, order
+        assert rel_l2(a, want) < tol, order
+        assert rel_l2(a, b) < tol, order
