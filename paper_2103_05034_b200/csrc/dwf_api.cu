@@ -415,7 +415,7 @@ static int launch_hop_t(dwf_ctx* h, const HopCall& k) {
     a.ax_a = (R)k.ax_a; a.ax_b = (R)k.ax_b; a.ax_c = (R)k.ax_c; a.g5_shift = (R)k.g5_shift;
     const int K = h->Ls / Prec<R>::VL;
     // tiled persistent stencil (dwf_tile.cuh): lattice made of whole tiles, compile-time Ls, a hop to do
-    const int TS = (k.mode != HM_SELF && tiled_ok(h)) ? h->tile_sites : 0;
+    const int TS = (k.mode != HM_SELF && tiled_ok(h) && h->V4h * (long long)k.nrhs < (1LL << 31)) ? h->tile_sites : 0;   // 32-bit block indices in the tiled kernel
     a.sg_shift = h->sg_shift;
     a.GS = TS ? TS : std::min(HOP_THREADS / 8, HOP_THREADS / K);                                   // sites per CTA
     a.ngroups = (h->V4h + a.GS - 1) / a.GS;

@@ -186,8 +186,11 @@ __device__ __forceinline__ void self_term(CV<float2> (&res)[12], const float4* _
             else { const CV<float2> o = unpack(ldg_nc(up_p + c * K)); ox_re = o.re.x; ox_im = o.im.x; }
             t.re = make_float2(own.re.y, ox_re); t.im = make_float2(own.im.y, ox_im); coef = coef_up;
         }
-        res[c].re = vfma2(coef, t.re, vfma(c_diag, own.re, res[c].re));
-        res[c].im = vfma2(coef, t.im, vfma(c_diag, own.im, res[c].im));
+        // the shifted-lane terms as scalar FMAs: no re-packing of (s-1 | s) pairs into aligned register pairs (2 MOVs per pair)
+        float2 rr = vfma(c_diag, own.re, res[c].re), ri = vfma(c_diag, own.im, res[c].im);
+        rr.x = fmaf(coef.x, t.re.x, rr.x); rr.y = fmaf(coef.y, t.re.y, rr.y);
+        ri.x = fmaf(coef.x, t.im.x, ri.x); ri.y = fmaf(coef.y, t.im.y, ri.y);
+        res[c].re = rr; res[c].im = ri;
     }
 }
 

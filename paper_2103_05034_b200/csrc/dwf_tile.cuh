@@ -243,14 +243,19 @@ hop_tile_kernel(const HopArgs<R> a) {
             const G* s_in = reinterpret_cast<const G*>(smem + TG::HDR + ib * TG::INT_STRIDE);
             const G* in = a.in_hop[pi] + k;
             // neighbour block: inside the tile -> shared memory, else global memory
+            // blk_index(n, r) = n + (n >> SH) * (nrhs - 1) * TS + r * TS in 32 bits (launch_hop_t checks V4h * nrhs < 2^31): the 64-bit
+            // form cost ~30 integer instructions per direction and thread
+            const unsigned nb_c1 = (unsigned)(a.nrhs - 1) << SH, nb_c2 = (unsigned)r << SH;
             auto nb = [&](int n) -> const G* {
-                if ((long long)(n >> SH) == gg) return s_in + (n & (TS - 1)) * BS + k;
-                return in + (size_t)blk_index(n, r, a.nrhs, SH) * BS;
+                const unsigned tn = (unsigned)n >> SH;
+                if (tn == (unsigned)gg) return s_in + ((unsigned)n & (TS - 1)) * BS + k;
+                return in + (size_t)((unsigned)n + tn * nb_c1 + nb_c2) * BS;
             };
             const G* q0 = nb(n0.x); const G* q1 = nb(n0.y); const G* q2 = nb(n0.z); const G* q3 = nb(n0.w);
             const G* q4 = nb(n1.x); const G* q5 = nb(n1.y); const G* q6 = nb(n1.z); const G* q7 = nb(n1.w);
             constexpr int SF = DAG ? +1 : -1;                  // projector sign on the forward hop
             mbar_wait(bar_int + ib, (NSTI == 2) ? (it >> 1) & 1 : it & 1);
+            {   // (the scope is deliberate: with it nvcc 12.9 spills 20 instead of 96 bytes in the G5+AXPBY variant, order-64 Chebyshev -5 %)
             tile_dir<0, SF, true >(acc, q0, K, u + 0 * 36);
             tile_dir<0, -SF, false>(acc, q1, K, u + 0 * 36);
             tile_dir<1, SF, true >(acc, q2, K, u + 1 * 36);
@@ -259,6 +264,7 @@ hop_tile_kernel(const HopArgs<R> a) {
             tile_dir<2, -SF, false>(acc, q5, K, u + 2 * 36);
             tile_dir<3, SF, true >(acc, q6, K, u + 3 * 36);
             tile_dir<3, -SF, false>(acc, q7, K, u + 3 * 36);
+            }
             // The last warp to finish with the shared-memory buffers of this item refills them: the interior with
             // item it+1, this small buffer with item it+2 (nobody waits: arrival is awaited through the mbarriers).
             auto release_buffers = [&]() {
@@ -352,19 +358,27 @@ hop_tile_kernel(const HopArgs<R> a) {
         int ko = k;
         if constexpr (G5) {
             ko = K - 1 - k;
+            // with the axpby epilogue its factor ax_a rides on the lane swap (two scalar multiplies into the swapped positions
+            // instead of two register moves and a packed multiply)
 #pragma unroll
             for (int c = 0; c < 12; c++) {
-                acc[c].re = vswap(acc[c].re); acc[c].im = vswap(acc[c].im);
-                if (c >= 6) { acc[c].re = vneg(acc[c].re); acc[c].im = vneg(acc[c].im); }
+                if constexpr (AXPBY) {
+                    const R sc = (c >= 6) ? -ax_a : ax_a;
+                    acc[c].re = vswapmul(sc, acc[c].re); acc[c].im = vswapmul(sc, acc[c].im);
+                } else {
+                    acc[c].re = vswap(acc[c].re); acc[c].im = vswap(acc[c].im);
+                    if (c >= 6) { acc[c].re = vneg(acc[c].re); acc[c].im = vneg(acc[c].im); }
+                }
             }
             // res = (H_DW + shift) in: the input at the OUTPUT location is lane group K-1-k of this thread's own (site, rhs) block,
             // the lines the self term has just read (L1 hits).  The factored Chebyshev step of dwf_api.cu x_step uses it.
             if (SELF && a.g5_shift != R(0)) {
                 const G* t = a.in_self[pi] + (size_t)blk * BS + ko;
+                const R sh = AXPBY ? ax_a * a.g5_shift : a.g5_shift;
 #pragma unroll
                 for (int c = 0; c < 12; c++) {
                     const CV<V> tt = unpack(ldg_nc(t + c * K));
-                    acc[c].re = vfma(a.g5_shift, tt.re, acc[c].re); acc[c].im = vfma(a.g5_shift, tt.im, acc[c].im);
+                    acc[c].re = vfma(sh, tt.re, acc[c].re); acc[c].im = vfma(sh, tt.im, acc[c].im);
                 }
             }
         }
@@ -372,8 +386,10 @@ hop_tile_kernel(const HopArgs<R> a) {
         if constexpr (AXPBY) {
             const G* y = a.y[pi] + obase;
             const G* z = a.z[pi] + obase;
+            if constexpr (!G5) {
 #pragma unroll
-            for (int c = 0; c < 12; c++) { acc[c].re = vmul(ax_a, acc[c].re); acc[c].im = vmul(ax_a, acc[c].im); }
+                for (int c = 0; c < 12; c++) { acc[c].re = vmul(ax_a, acc[c].re); acc[c].im = vmul(ax_a, acc[c].im); }
+            }
             if (a.ax_b != R(0)) {                              // a zero coefficient means "operand absent": it is not read
 #pragma unroll
                 for (int c = 0; c < 12; c++) {

@@ -26,6 +26,8 @@ __device__ __forceinline__ float2 vfnma(float s, float2 b, float2 c) { return __
 // lane-wise coefficient pair
 __device__ __forceinline__ float2 vfma2(float2 s, float2 b, float2 c) { return __ffma2_rn(s, b, c); }
 __device__ __forceinline__ float2 vswap(float2 a) { return make_float2(a.y, a.x); }
+// s * (lanes swapped): two scalar multiplies that write the swapped positions (no register moves)
+__device__ __forceinline__ float2 vswapmul(float s, float2 a) { return make_float2(s * a.y, s * a.x); }
 
 // ---- fp64 (one lane) ----
 __device__ __forceinline__ double vzero(double) { return 0.0; }
@@ -37,6 +39,7 @@ __device__ __forceinline__ double vfma(double s, double b, double c) { return fm
 __device__ __forceinline__ double vfnma(double s, double b, double c) { return fma(-s, b, c); }
 __device__ __forceinline__ double vfma2(double s, double b, double c) { return fma(s, b, c); }
 __device__ __forceinline__ double vswap(double a) { return a; }
+__device__ __forceinline__ double vswapmul(double s, double a) { return s * a; }
 
 // complex number whose re and im are lane vectors
 template <typename V> struct CV { V re, im; };
