@@ -366,8 +366,8 @@ hop_tile_kernel(const HopArgs<R> a) {
                     const R sc = (c >= 6) ? -ax_a : ax_a;
                     acc[c].re = vswapmul(sc, acc[c].re); acc[c].im = vswapmul(sc, acc[c].im);
                 } else {
-                    acc[c].re = vswap(acc[c].re); acc[c].im = vswap(acc[c].im);
-                    if (c >= 6) { acc[c].re = vneg(acc[c].re); acc[c].im = vneg(acc[c].im); }
+                    const R sc = (c >= 6) ? R(-1) : R(1);          // exact; scalar multiplies into the swapped positions: MOV 173 -> 112
+                    acc[c].re = vswapmul(sc, acc[c].re); acc[c].im = vswapmul(sc, acc[c].im);
                 }
             }
             // res = (H_DW + shift) in: the input at the OUTPUT location is lane group K-1-k of this thread's own (site, rhs) block,
