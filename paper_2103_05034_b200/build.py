@@ -22,7 +22,10 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--split-compile=0",
+        # No --split-compile: the way nvcc partitions the module over threads changes the register allocation and instruction
+        # count of the stencil kernels from build to build (order-64 Chebyshev 477 / 482 / 490 ms for three builds of one source,
+        # DESIGN.md sec. 5.1); the single-partition compile is the fastest of them and reproducible (2.5 min instead of 1.2).
+        cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
                "-Xcompiler", "-fPIC", "-shared", "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")

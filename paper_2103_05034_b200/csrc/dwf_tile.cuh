@@ -255,7 +255,6 @@ hop_tile_kernel(const HopArgs<R> a) {
             const G* q4 = nb(n1.x); const G* q5 = nb(n1.y); const G* q6 = nb(n1.z); const G* q7 = nb(n1.w);
             constexpr int SF = DAG ? +1 : -1;                  // projector sign on the forward hop
             mbar_wait(bar_int + ib, (NSTI == 2) ? (it >> 1) & 1 : it & 1);
-            {   // (the scope is deliberate: with it nvcc 12.9 spills 20 instead of 96 bytes in the G5+AXPBY variant, order-64 Chebyshev -5 %)
             tile_dir<0, SF, true >(acc, q0, K, u + 0 * 36);
             tile_dir<0, -SF, false>(acc, q1, K, u + 0 * 36);
             tile_dir<1, SF, true >(acc, q2, K, u + 1 * 36);
@@ -264,7 +263,6 @@ hop_tile_kernel(const HopArgs<R> a) {
             tile_dir<2, -SF, false>(acc, q5, K, u + 2 * 36);
             tile_dir<3, SF, true >(acc, q6, K, u + 3 * 36);
             tile_dir<3, -SF, false>(acc, q7, K, u + 3 * 36);
-            }
             // The last warp to finish with the shared-memory buffers of this item refills them: the interior with
             // item it+1, this small buffer with item it+2 (nobody waits: arrival is awaited through the mbarriers).
             auto release_buffers = [&]() {
