@@ -304,7 +304,13 @@ hop_tile_kernel(const HopArgs<R> a) {
                 __syncthreads();                               // every warp is done reading the interior
 #pragma unroll
                 for (int c = 0; c < 12; c++) s_t[(ls * 12 + c) * (K + 1) + k] = pack(acc[c]);
-                __syncthreads();
+                // When K divides 32 a site's rows are written and read back by threads of ONE warp: each warp solves the rows of its
+                // own sites (32/K sites x 24 tasks) and the two hand-overs are warp barriers, not CTA barriers.
+                constexpr bool WARP_LOCAL = (32 % K == 0);
+                constexpr int TASKS = WARP_LOCAL ? (32 / K) * 24 : TS * 24;        // per warp | per CTA
+                constexpr int TSTEP = WARP_LOCAL ? 32 : TG::THREADS;
+                const int task0 = WARP_LOCAL ? (int)(threadIdx.x >> 5) * TASKS : 0;
+                if constexpr (WARP_LOCAL) __syncwarp(); else __syncthreads();
                 const R kappa = a.moo_kappa, v0scale = a.moo_v0scale, mass = a.mass;
                 G* obase_t = a.out[pi] + (size_t)blk_index(gg * TS, r, a.nrhs, SH) * BS;   // the tile's blocks are one run
                 // task = (row, real | imaginary part): TS*24 tasks = a whole number of passes of the CTA (3 for 32 sites x 256
@@ -312,7 +318,8 @@ hop_tile_kernel(const HopArgs<R> a) {
                 // and writes whole 16-byte groups
                 using H = typename std::conditional<VL == 2, float2, double>::type;        // one part of a group
                 const H* s_h = reinterpret_cast<const H*>(s_t);
-                for (int task = threadIdx.x; task < TS * 24; task += TG::THREADS) {
+                for (int tk = WARP_LOCAL ? (int)(threadIdx.x & 31) : (int)threadIdx.x; tk < TASKS; tk += TSTEP) {
+                    const int task = task0 + tk;
                     const int row = task >> 1, part = task & 1;
                     const int c = row % 12;
                     const bool down = DAG ? (c >= 6) : (c < 6);
@@ -341,7 +348,7 @@ hop_tile_kernel(const HopArgs<R> a) {
                         s_w[(row * (K + 1) + (down ? kk : K - 1 - kk)) * 2 + part] = g;
                     }
                 }
-                __syncthreads();
+                if constexpr (WARP_LOCAL) __syncwarp(); else __syncthreads();
                 // ... and out in the lane layout: the same whole-line streaming stores as every other epilogue (storing the rows
                 // straight from the tasks costs 16 half-used sectors per warp instruction: Schur K1 91 us instead of 7x us)
                 {
